@@ -1,0 +1,151 @@
+/* mg.h — C ABI of the B200 (sm_100a) tree-level matrix-element library.
+ *
+ * The library implements the data-parallel hot path of arXiv 2106.12631:
+ *   random numbers -> RAMBO momenta -> helicity amplitudes -> colour-summed |M|^2 ("sigmaKin"),
+ * PAPER.md:78 (§3, the three components), PAPER.md:92 (§4, data flow), PAPER.md:33/:35 (§2, the
+ * ME algorithm).  Stateless functions over a basket of events reading/writing fixed-size C arrays
+ * (PAPER.md:94, :98); memory is allocated by the caller before the first and freed after the last
+ * iteration.  Readings of the paper's silences are numbered R1.. in DESIGN.md.
+ *
+ * Conventions common to every call
+ *  - Return value: 0 (MG_OK) or a negative MG_E* code; no exceptions, no abort().  n == 0 is a no-op.
+ *  - d_* pointers are DEVICE memory owned by the caller; h_* pointers are HOST memory owned by the
+ *    caller.  The library allocates nothing per call except where stated, and keeps no reference
+ *    to a caller buffer after the work it enqueued has finished.
+ *  - `stream` is a cudaStream_t passed as void* (NULL = default stream).  Calls taking only d_*
+ *    buffers are asynchronous on that stream unless stated otherwise.
+ *  - Element type of every floating-point buffer = the precision of the handle (double for
+ *    MG_FP64, float for MG_FP32).
+ *  - Layout: structure of arrays, EVENT INDEX FASTEST, row stride `ld` elements (ld >= n):
+ *        rnd     [(i_final*4 + k ) * ld + e]    k  = 0..3  (rho_1..rho_4 of final particle i_final)
+ *        momenta [(i_par  *4 + mu) * ld + e]    mu = 0..3  (E, px, py, pz), GeV
+ *        me, ps_weight, event_weight [e]
+ *    Particle order (R9): beams first, then the final state as the process is written:
+ *        MG_EEMUMU: e+ e- mu+ mu-      MG_GGTT..: g g t t~ [g [g]]
+ *    Beams (R5): particle 0 = (sqrt_s/2,0,0,+sqrt_s/2), particle 1 = (sqrt_s/2,0,0,-sqrt_s/2).
+ *  - Helicity-combination index: bit k of the index = helicity of particle k (0 <-> -1, 1 <-> +1).
+ *  - Determinism: the result for event e depends only on (seed, first_event + e, params), never on
+ *    n, ld, the launch shape or the stream.
+ *  - There is no CPU fallback: every entry point that computes needs a CUDA device of compute
+ *    capability 10.x and fails with MG_ECUDA otherwise.
+ */
+#ifndef MG_B200_H
+#define MG_B200_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct mg_process mg_process; /* opaque; owns constant tables and small device scratch */
+
+enum { MG_EEMUMU = 0, MG_GGTT = 1, MG_GGTTG = 2, MG_GGTTGG = 3 };
+enum { MG_FP64 = 0, MG_FP32 = 1 };
+enum { MG_OK = 0, MG_EINVAL = -1, MG_EPARAM = -2, MG_ECUDA = -3, MG_ENOMEM = -4 };
+/* stages for mg_flops_per_event / mg_bytes_per_event */
+enum { MG_STAGE_RNG = 0, MG_STAGE_RAMBO = 1, MG_STAGE_SIGMAKIN = 2, MG_STAGE_GENERATE = 3 };
+
+/* Physics and run parameters (BASELINE.json configs; readings R12-R15). */
+typedef struct {
+  int32_t process;     /* MG_EEMUMU .. MG_GGTTGG */
+  int32_t precision;   /* MG_FP64 | MG_FP32 */
+  int32_t device;      /* CUDA device ordinal */
+  int32_t reserved;    /* must be 0 */
+  double sqrt_s;       /* GeV; 1500 */
+  double alpha_em_inv; /* 132.507            (MG_EEMUMU) */
+  double mZ, gammaZ;   /* 91.188, 2.441 GeV  (MG_EEMUMU) */
+  double mW;           /* 80.419 GeV: sin^2(theta_W) = 1 - mW^2/mZ^2 (R14) */
+  double mt;           /* 173 GeV            (MG_GGTT..); the top width is 0 (R12) */
+  double alpha_s;      /* 0.118              (MG_GGTT..) */
+} mg_params;
+
+/* Fills *out with the BASELINE.json parameter set for (process, precision), device 0. */
+int mg_default_params(int process, int precision, mg_params* out);
+
+/* Creates a process handle: validates params (MG_EPARAM if sum of final masses >= sqrt_s or a
+ * parameter is not finite/positive), selects the device, allocates a few KB of device scratch.
+ * The helicity mask starts as "all helicities" (no filtering).  PAPER.md:136 (constants),
+ * PAPER.md:112 (allocation outside the event loop). */
+int mg_init_process(const mg_params* params, mg_process** out);
+int mg_free_process(mg_process* p);
+
+/* Static facts of the process (Fig. 3: 4/4/5/6 external particles; BASELINE configs). */
+int mg_n_external(const mg_process* p);     /* 4,4,5,6 */
+int mg_n_final(const mg_process* p);        /* 2,2,3,4 */
+int mg_n_helicities(const mg_process* p);   /* 16,16,32,64 */
+int mg_n_colour_flows(const mg_process* p); /* 1,2,6,24 */
+int mg_n_diagrams(const mg_process* p);     /* 2,3,16,123 */
+int mg_n_amplitudes(const mg_process* p);   /* 2,3,18,159 (a 4-gluon vertex carries 3 structures) */
+int mg_me_denominator(const mg_process* p); /* 4,256,256,512 (R11) */
+/* Colour matrix C (n_flows x n_flows, row-major, doubles) copied to host memory `out`. */
+int mg_colour_matrix(const mg_process* p, double* h_out);
+/* Smallest row stride the library recommends for n events (n rounded up to a multiple of 32). */
+int64_t mg_padded_stride(int64_t n);
+
+/* A1: Philox4x32-10 words (R1, R2).  d_words[(i_final*4+k)*ld + e] = word k of
+ * Philox(counter = (event_lo, event_hi, i_final, 0), key = (seed_lo, seed_hi)), event =
+ * first_event + e.  uint32 regardless of precision. */
+int mg_rng_words(mg_process* p, uint64_t seed, uint64_t first_event, int64_t n, int64_t ld,
+                 uint32_t* d_words, void* stream);
+/* A1+A2: the same words mapped to uniforms in (0,1) (R3): FP64 (x+0.5)*2^-32, FP32 ((x>>9)+0.5)*2^-23. */
+int mg_rng(mg_process* p, uint64_t seed, uint64_t first_event, int64_t n, int64_t ld,
+           void* d_rnd, void* stream);
+
+/* A3+A4: RAMBO (Kleiss-Stirling-Ellis; R5-R8).  Reads rnd[4*n_final][ld], writes
+ * momenta[4*n_external][ld] (beams included) and the phase-space weight ps_weight[n] (nullable).
+ * sqrt_s and masses come from the handle. */
+int mg_rambo(mg_process* p, const void* d_rnd, int64_t n, int64_t ld,
+             void* d_momenta, void* d_ps_weight, void* stream);
+
+/* A1-A4 fused: uniforms never touch HBM.  Same results as mg_rng + mg_rambo. */
+int mg_generate(mg_process* p, uint64_t seed, uint64_t first_event, int64_t n, int64_t ld,
+                void* d_momenta, void* d_ps_weight, void* stream);
+
+/* A12: good-helicity filter (R16).  Evaluates every helicity combination on the
+ * first probe_n events of d_momenta (1 <= probe_n <= n... the caller guarantees probe_n events are
+ * present), marks h good iff max_e |M|^2_h / sum_h' |M|^2_h' > 1e-10, returns the mask in
+ * *h_out_mask (nullable) AND installs it in the handle.  Synchronises the stream.  Allocates and
+ * frees probe_n * n_helicities elements of device scratch. */
+int mg_filter_helicities(mg_process* p, const void* d_momenta, int64_t probe_n, int64_t ld,
+                         uint64_t* h_out_mask, void* stream);
+int mg_set_helicity_mask(mg_process* p, uint64_t mask); /* bits above n_helicities are ignored */
+int mg_get_helicity_mask(const mg_process* p, uint64_t* h_out_mask);
+
+/* A5-A11 (+A13): sigmaKin.  me[e] = (1/denominator) * sum over the
+ * helicities in the handle's mask of J^dagger C J.  If both d_ps_weight and d_event_weight are
+ * non-NULL also writes event_weight[e] = ps_weight[e] * me[e] (R18). */
+int mg_sigmakin(mg_process* p, const void* d_momenta, int64_t n, int64_t ld, void* d_me,
+                const void* d_ps_weight, void* d_event_weight, void* stream);
+
+/* Diagnostic form of A5-A10: |M|^2 of EVERY helicity combination (mask ignored, no 1/denominator):
+ * d_me_hel[h*ld + e].  Used by the filter and by the parity tests (per-helicity |M|^2 is
+ * convention independent, R22). */
+int mg_sigmakin_per_helicity(mg_process* p, const void* d_momenta, int64_t n, int64_t ld,
+                             void* d_me_hel, void* stream);
+
+/* Host-buffer forms (the end-to-end path; "copy ... to the host").  Synchronous.
+ * mg_sigmakin_host: copies h_momenta [4*n_external][ld] to the device, runs sigmaKin, copies
+ * h_me[n] back.  mg_run_host: runs A1-A13 for events [first_event, first_event+n) on the device and
+ * copies momenta (nullable), ps_weight (nullable) and me to the host.  Device scratch is grown
+ * inside the handle on first use and reused. */
+int mg_sigmakin_host(mg_process* p, const void* h_momenta, int64_t n, int64_t ld, void* h_me);
+int mg_run_host(mg_process* p, uint64_t seed, uint64_t first_event, int64_t n, int64_t ld,
+                void* h_momenta, void* h_ps_weight, void* h_me);
+
+/* Algorithmic work per event of one stage: explicit
+ * tallies emitted with the kernels; flops for MG_STAGE_SIGMAKIN are per event for the CURRENT
+ * helicity mask (FMA = 2). */
+int64_t mg_flops_per_event(const mg_process* p, int stage);
+int64_t mg_bytes_per_event(const mg_process* p, int stage);
+/* Duration in ms of the dominant kernel of the last mg_*_host call, measured with CUDA events on
+ * the library's stream (0 if none). */
+double mg_last_kernel_ms(const mg_process* p);
+
+const char* mg_strerror(int code);
+const char* mg_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* MG_B200_H */

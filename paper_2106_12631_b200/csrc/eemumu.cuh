@@ -1,0 +1,76 @@
+// eemumu.cuh — sigmaKin for e+ e- -> mu+ mu- (photon + Z), hand-written in the routine order of
+// PAPER.md:33 (Fig. 1 caption): external wavefunctions (IXXXXX/OXXXXX) for the four fermions, then
+//   FFV1P0_3 : photon off-shell wavefunction from the e+ e- gamma vertex (incl. propagator 1/s)
+//   FFV1_0   : amplitude of diagram (a) from the gamma mu mu vertex
+//   FFV2_4_3 : Z off-shell wavefunction from the e+ e- Z vertex (incl. propagator)
+//   FFV2_4_0 : amplitude of diagram (b) from the Z mu mu vertex
+// "The two amplitudes are added to each other, their sum is squared, and the result is averaged
+// over all valid helicity combinations".
+//
+// Rules (R13-R15): l l gamma: i e gamma^mu;  l l Z: i e/(sW cW) gamma^mu (gL PL + gR PR);
+// photon propagator -i g/q^2;  Z propagator -i (g - q q/mZ^2)/(q^2 - mZ^2 + i mZ GammaZ).  Both diagrams
+// carry the same overall factor i^2 (-i) = i, dropped.  Massless leptons: the chirality block that
+// vanishes is an exact zero, so exactly 4 of the 16 helicity combinations are non-zero.
+// Particle order (R9): 0 = e+, 1 = e-, 2 = mu+, 3 = mu-.
+#pragma once
+#include "helas.cuh"
+
+namespace mg {
+
+struct Eemumu {
+  static constexpr int NHEL = 16;
+  static constexpr int NPAR = 4;
+  template <class T> struct Event { Mom<T> p[4]; Mom<T> q; T is; cx<T> bw; };
+
+  template <class T> static MG_HD void finish(Event<T>& ev, const Consts& k) {
+    ev.q = ev.p[0] + ev.p[1];
+    const T s = mdot(ev.q, ev.q);
+    ev.is = (T)1 / s;
+    // 1/(s - mZ^2 + i mZ GZ)
+    const T dr = s - (T)k.mZ2, di = (T)k.mZgZ;
+    const T inv = (T)1 / fma_<T>(dr, dr, di * di);
+    ev.bw = cx<T>(dr * inv, -di * inv);
+  }
+
+  template <class T> static MG_HD T helicity(const Event<T>& ev, int ihel, const Consts& k) {
+    const int h0 = (ihel & 1) ? 1 : -1, h1 = (ihel & 2) ? 1 : -1, h2 = (ihel & 4) ? 1 : -1, h3 = (ihel & 8) ? 1 : -1;
+    // OXXXXX / IXXXXX: incoming e+ -> vbar, incoming e- -> u, outgoing mu+ -> v, outgoing mu- -> ubar
+    const Spinor<T> vbar_ep = bar(spinor_v<T>(ev.p[0], (T)0, h0));
+    const Spinor<T> u_em = spinor_u<T>(ev.p[1], (T)0, h1);
+    const Spinor<T> v_mup = spinor_v<T>(ev.p[2], (T)0, h2);
+    const Spinor<T> ubar_mum = bar(spinor_u<T>(ev.p[3], (T)0, h3));
+    const T e = (T)k.ee, gzl = (T)k.gzl, gzr = (T)k.gzr;
+
+    // chirality-split current of the electron line: J_R = a sigma^mu psi_R, J_L = b sigmabar^mu psi_L
+    Spinor<T> onlyR = vbar_ep, onlyL = vbar_ep;
+    onlyR.r[0] = onlyR.r[1] = cx<T>(0, 0);   // keep a (couples to psi_R)
+    onlyL.l[0] = onlyL.l[1] = cx<T>(0, 0);   // keep b (couples to psi_L)
+    const Vec4<T> JR = ff_current(onlyR, u_em);
+    const Vec4<T> JL = ff_current(onlyL, u_em);
+
+    // FFV1P0_3: A^mu = e (J_L + J_R)^mu / s
+    Vec4<T> A;
+#pragma unroll
+    for (int mu = 0; mu < 4; ++mu) A.v[mu] = (e * ev.is) * (JL.v[mu] + JR.v[mu]);
+    // FFV1_0: e ubar Aslash v
+    const cx<T> amp_a = e * ffv_amp(ubar_mum, A, v_mup);
+
+    // FFV2_4_3: Z^mu = [Jz^mu - q^mu (Jz.q)/mZ^2] / (s - mZ^2 + i mZ GZ),  Jz = gzl J_L + gzr J_R
+    Vec4<T> Jz;
+#pragma unroll
+    for (int mu = 0; mu < 4; ++mu) Jz.v[mu] = rfma(gzr, JR.v[mu], gzl * JL.v[mu]);
+    const cx<T> jq = ((T)1 / (T)k.mZ2) * mdot(Jz, ev.q);
+    Vec4<T> Z;
+#pragma unroll
+    for (int mu = 0; mu < 4; ++mu) Z.v[mu] = ev.bw * rfma(-ev.q.v[mu], jq, Jz.v[mu]);
+    // FFV2_4_0: ubar Zslash (gzl PL + gzr PR) v = gzl b.Sb(Z) v_L + gzr a.S(Z) v_R
+    const Spinor<T> zv = slash_col(slash_parts(Z), v_mup);   // (S(Z) v_R ; Sb(Z) v_L)
+    cx<T> aR = cfma(ubar_mum.l[1], zv.l[1], ubar_mum.l[0] * zv.l[0]);
+    cx<T> bL = cfma(ubar_mum.r[1], zv.r[1], ubar_mum.r[0] * zv.r[0]);
+    const cx<T> amp_b = rfma(gzr, aR, gzl * bL);
+
+    return norm2(amp_a + amp_b);
+  }
+};
+
+}  // namespace mg

@@ -1,0 +1,40 @@
+// me_tables.cu — generated tables (flop tallies, colour matrices) behind mg_flops_per_event / mg_colour_matrix.
+#include "mg_internal.h"
+#include "gen_tables.cuh"
+
+namespace mg {
+
+// e+ e- -> mu+ mu-: hand tally of eemumu.cuh: 4 spinors (4 x 30),
+// 2 chirality currents (2 x 72), photon wavefunction (24), FFV1_0 (94 + 2), Z wavefunction (16 + 14 + 2 + 40),
+// FFV2_4_0 (8 + 56 + 28 + 6), sum and square (2 + 3).
+static const int kFlopsPerHelicity_ee = 4 * 30 + 2 * 72 + 24 + 96 + 72 + 98 + 5;
+static const int kFlopsFixed_ee = 4 + 7 + 1 + 1 + 4 + 3;
+
+int64_t me_flops_per_helicity(int process) {
+  switch (process) {
+    case MG_EEMUMU: return kFlopsPerHelicity_ee;
+    case MG_GGTT: return kFlopsPerHelicity_2;
+    case MG_GGTTG: return kFlopsPerHelicity_3;
+    case MG_GGTTGG: return kFlopsPerHelicity_4;
+  }
+  return 0;
+}
+int64_t me_flops_per_event_fixed(int process) {
+  switch (process) {
+    case MG_EEMUMU: return kFlopsFixed_ee;
+    case MG_GGTT: return kFlopsFixed_2;
+    case MG_GGTTG: return kFlopsFixed_3;
+    case MG_GGTTGG: return kFlopsFixed_4;
+  }
+  return 0;
+}
+const int* me_colour_numerators(int process, int* den) {
+  switch (process) {
+    case MG_GGTT: *den = kColourDen_2; return kColourNum_2;
+    case MG_GGTTG: *den = kColourDen_3; return kColourNum_3;
+    case MG_GGTTGG: *den = kColourDen_4; return kColourNum_4;
+  }
+  return nullptr;
+}
+
+}  // namespace mg

@@ -1,0 +1,355 @@
+// mg_api.cu — the C ABI of include/mg.h: argument checking, handle, stream/device plumbing,
+// host-buffer (end-to-end) forms.  Every compute step is a kernel launch in rng_rambo.cu / me_*.cu;
+// nothing is computed on the host (no CPU fallback).
+#include <math.h>
+#include <new>
+#include <string.h>
+#include "mg_internal.h"
+
+using namespace mg;
+
+namespace {
+
+struct ProcInfo { int n_ext, n_final, n_hel, n_flows, n_diag, n_amp, denom; };
+const ProcInfo kInfo[4] = {
+    {4, 2, 16, 1, 2, 2, 4},        // e+e- -> mu+mu-     
+    {4, 2, 16, 2, 3, 3, 256},      // gg -> tt~          (BASELINE.json configs[2])
+    {5, 3, 32, 6, 16, 18, 256},    // gg -> tt~g         (configs[3])
+    {6, 4, 64, 24, 123, 159, 512}, // gg -> tt~gg        (configs[4])
+};
+
+inline bool valid_handle(const mg_process* p) { return p != nullptr; }
+inline size_t elem(const mg_process* p) { return p->par.precision == MG_FP64 ? 8 : 4; }
+inline bool aligned(const void* q, size_t a) { return ((uintptr_t)q % a) == 0; }
+
+struct DeviceGuard {
+  int prev = -1; bool ok = true;
+  explicit DeviceGuard(int dev) {
+    if (cudaGetDevice(&prev) != cudaSuccess) { ok = false; return; }
+    if (prev != dev && cudaSetDevice(dev) != cudaSuccess) ok = false;
+  }
+  ~DeviceGuard() { if (prev >= 0) cudaSetDevice(prev); }
+};
+
+int cuda_rc(cudaError_t e) { return e == cudaSuccess ? MG_OK : (e == cudaErrorMemoryAllocation ? MG_ENOMEM : MG_ECUDA); }
+
+double rambo_w0(int n, double sqrt_s) {  // (pi/2)^(n-1) s^(n-2) / ((n-1)!(n-2)!) (2 pi)^(4-3n)   (north_star)
+  const double pi = 3.14159265358979323846;
+  double w = pow(pi / 2, n - 1) * pow(sqrt_s * sqrt_s, n - 2) * pow(2 * pi, 4 - 3 * n);
+  for (int i = 2; i <= n - 1; ++i) w /= i;
+  for (int i = 2; i <= n - 2; ++i) w /= i;
+  return w;
+}
+
+int ensure_scratch(mg_process* p, size_t dev_bytes, size_t host_bytes) {
+  if (dev_bytes > p->scratch_bytes) {
+    if (p->d_scratch) cudaFree(p->d_scratch);
+    p->d_scratch = nullptr; p->scratch_bytes = 0;
+    cudaError_t e = cudaMalloc(&p->d_scratch, dev_bytes);
+    if (e != cudaSuccess) { cudaGetLastError(); return MG_ENOMEM; }
+    p->scratch_bytes = dev_bytes;
+  }
+  (void)host_bytes;
+  return MG_OK;
+}
+
+cudaError_t launch_me(const mg_process* p, const MeArgs& a, cudaStream_t s) {
+  switch (p->par.process) {
+    case MG_EEMUMU: return launch_me_eemumu(p, a, s);
+    case MG_GGTT: return launch_me_ggtt(p, a, s);
+    case MG_GGTTG: return launch_me_ggttg(p, a, s);
+    case MG_GGTTGG: return launch_me_ggttgg(p, a, s);
+  }
+  return cudaErrorInvalidValue;
+}
+
+int check_soa(const mg_process* p, const void* ptr, int64_t n, int64_t ld) {
+  if (!valid_handle(p) || n < 0) return MG_EINVAL;
+  if (n == 0) return MG_OK;
+  if (ptr == nullptr || ld < n || !aligned(ptr, elem(p))) return MG_EINVAL;
+  return MG_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int mg_default_params(int process, int precision, mg_params* out) {
+  if (!out || process < 0 || process > 3 || (precision != MG_FP64 && precision != MG_FP32)) return MG_EINVAL;
+  memset(out, 0, sizeof(*out));
+  out->process = process; out->precision = precision; out->device = 0;
+  out->sqrt_s = 1500.0; out->alpha_em_inv = 132.507; out->mZ = 91.188; out->gammaZ = 2.441; out->mW = 80.419;
+  out->mt = 173.0; out->alpha_s = 0.118;
+  return MG_OK;
+}
+
+int mg_init_process(const mg_params* par, mg_process** out) {
+  if (!par || !out) return MG_EINVAL;
+  *out = nullptr;
+  if (par->process < 0 || par->process > 3 || (par->precision != MG_FP64 && par->precision != MG_FP32) || par->reserved != 0 || par->device < 0)
+    return MG_EINVAL;
+  const ProcInfo& I = kInfo[par->process];
+  auto pos = [](double x) { return isfinite(x) && x > 0; };
+  if (!pos(par->sqrt_s)) return MG_EPARAM;
+  if (par->process == MG_EEMUMU) {
+    if (!pos(par->alpha_em_inv) || !pos(par->mZ) || !pos(par->mW) || !isfinite(par->gammaZ) || par->gammaZ < 0 || par->mW >= par->mZ) return MG_EPARAM;
+  } else {
+    if (!pos(par->mt) || !pos(par->alpha_s) || 2 * par->mt >= par->sqrt_s) return MG_EPARAM;
+  }
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || par->device >= ndev) { cudaGetLastError(); return MG_ECUDA; }
+  cudaDeviceProp prop;
+  if (cudaGetDeviceProperties(&prop, par->device) != cudaSuccess || prop.major != 10) { cudaGetLastError(); return MG_ECUDA; }
+
+  mg_process* p = new (std::nothrow) mg_process();
+  if (!p) return MG_ENOMEM;
+  memset(p, 0, sizeof(*p));
+  p->par = *par;
+  p->n_ext = I.n_ext; p->n_final = I.n_final; p->n_hel = I.n_hel; p->n_flows = I.n_flows;
+  p->n_diag = I.n_diag; p->n_amp = I.n_amp; p->denom = I.denom;
+  p->hel_mask = I.n_hel == 64 ? ~0ull : ((1ull << I.n_hel) - 1);
+  Consts& k = p->k;
+  const double pi = 3.14159265358979323846;
+  k.sqrt_s = par->sqrt_s;
+  for (int i = 0; i < 4; ++i) k.mass[i] = 0;
+  k.w0 = rambo_w0(I.n_final, par->sqrt_s);
+  if (par->process == MG_EEMUMU) {
+    const double sw2 = 1 - (par->mW * par->mW) / (par->mZ * par->mZ), cw2 = 1 - sw2;   // R14
+    k.ee = sqrt(4 * pi / par->alpha_em_inv);                                           // R15
+    const double gz = k.ee / sqrt(sw2 * cw2);
+    k.gzl = gz * (-0.5 + sw2); k.gzr = gz * sw2;
+    k.mZ = par->mZ; k.mZ2 = par->mZ * par->mZ; k.mZgZ = par->mZ * par->gammaZ;
+    k.me_norm = 1.0 / I.denom;
+  } else {
+    k.mass[0] = k.mass[1] = par->mt; k.mt = par->mt;
+    k.gs = sqrt(4 * pi * par->alpha_s);                                                // R15
+    const int ng = I.n_ext - 2;
+    k.me_norm = pow(4 * pi * par->alpha_s, ng) / I.denom;                              // g_s^(2 n_g) / denominator
+  }
+  DeviceGuard g(par->device);
+  if (!g.ok || cudaStreamCreateWithFlags(&p->own_stream, cudaStreamNonBlocking) != cudaSuccess ||
+      cudaEventCreate(&p->ev0) != cudaSuccess || cudaEventCreate(&p->ev1) != cudaSuccess) {
+    cudaGetLastError(); delete p; return MG_ECUDA;
+  }
+  *out = p;
+  return MG_OK;
+}
+
+int mg_free_process(mg_process* p) {
+  if (!p) return MG_OK;
+  DeviceGuard g(p->par.device);
+  if (p->d_scratch) cudaFree(p->d_scratch);
+  if (p->h_pinned) cudaFreeHost(p->h_pinned);
+  if (p->ev0) cudaEventDestroy(p->ev0);
+  if (p->ev1) cudaEventDestroy(p->ev1);
+  if (p->own_stream) cudaStreamDestroy(p->own_stream);
+  delete p;
+  return MG_OK;
+}
+
+int mg_n_external(const mg_process* p) { return p ? p->n_ext : MG_EINVAL; }
+int mg_n_final(const mg_process* p) { return p ? p->n_final : MG_EINVAL; }
+int mg_n_helicities(const mg_process* p) { return p ? p->n_hel : MG_EINVAL; }
+int mg_n_colour_flows(const mg_process* p) { return p ? p->n_flows : MG_EINVAL; }
+int mg_n_diagrams(const mg_process* p) { return p ? p->n_diag : MG_EINVAL; }
+int mg_n_amplitudes(const mg_process* p) { return p ? p->n_amp : MG_EINVAL; }
+int mg_me_denominator(const mg_process* p) { return p ? p->denom : MG_EINVAL; }
+int64_t mg_padded_stride(int64_t n) { return n <= 0 ? 0 : (n + 31) / 32 * 32; }
+
+int mg_colour_matrix(const mg_process* p, double* h_out) {
+  if (!p || !h_out) return MG_EINVAL;
+  if (p->par.process == MG_EEMUMU) { h_out[0] = 1.0; return MG_OK; }
+  int den = 1;
+  const int* num = me_colour_numerators(p->par.process, &den);
+  if (!num) return MG_EINVAL;
+  for (int i = 0; i < p->n_flows * p->n_flows; ++i) h_out[i] = (double)num[i] / den;
+  return MG_OK;
+}
+
+int mg_rng_words(mg_process* p, uint64_t seed, uint64_t first_event, int64_t n, int64_t ld, uint32_t* d_words, void* stream) {
+  if (!valid_handle(p) || n < 0) return MG_EINVAL;
+  if (n == 0) return MG_OK;
+  if (!d_words || ld < n || !aligned(d_words, 4)) return MG_EINVAL;
+  DeviceGuard g(p->par.device); if (!g.ok) return MG_ECUDA;
+  return cuda_rc(launch_rng_words(p, seed, first_event, n, ld, d_words, (cudaStream_t)stream));
+}
+
+int mg_rng(mg_process* p, uint64_t seed, uint64_t first_event, int64_t n, int64_t ld, void* d_rnd, void* stream) {
+  int rc = check_soa(p, d_rnd, n, ld); if (rc != MG_OK || n == 0) return rc;
+  DeviceGuard g(p->par.device); if (!g.ok) return MG_ECUDA;
+  return cuda_rc(launch_rng(p, seed, first_event, n, ld, d_rnd, (cudaStream_t)stream));
+}
+
+int mg_rambo(mg_process* p, const void* d_rnd, int64_t n, int64_t ld, void* d_momenta, void* d_ps_weight, void* stream) {
+  int rc = check_soa(p, d_rnd, n, ld); if (rc != MG_OK || n == 0) return rc;
+  rc = check_soa(p, d_momenta, n, ld); if (rc != MG_OK) return rc;
+  if (d_ps_weight && !aligned(d_ps_weight, elem(p))) return MG_EINVAL;
+  DeviceGuard g(p->par.device); if (!g.ok) return MG_ECUDA;
+  return cuda_rc(launch_rambo(p, d_rnd, n, ld, d_momenta, d_ps_weight, (cudaStream_t)stream));
+}
+
+int mg_generate(mg_process* p, uint64_t seed, uint64_t first_event, int64_t n, int64_t ld, void* d_momenta, void* d_ps_weight, void* stream) {
+  int rc = check_soa(p, d_momenta, n, ld); if (rc != MG_OK || n == 0) return rc;
+  if (d_ps_weight && !aligned(d_ps_weight, elem(p))) return MG_EINVAL;
+  DeviceGuard g(p->par.device); if (!g.ok) return MG_ECUDA;
+  return cuda_rc(launch_generate(p, seed, first_event, n, ld, d_momenta, d_ps_weight, (cudaStream_t)stream));
+}
+
+int mg_sigmakin(mg_process* p, const void* d_momenta, int64_t n, int64_t ld, void* d_me, const void* d_ps_weight, void* d_event_weight, void* stream) {
+  int rc = check_soa(p, d_momenta, n, ld); if (rc != MG_OK || n == 0) return rc;
+  if (!d_me || !aligned(d_me, elem(p))) return MG_EINVAL;
+  MeArgs a{d_momenta, n, ld, d_me, nullptr, nullptr, nullptr, p->hel_mask};
+  if (d_ps_weight && d_event_weight) { a.psw = d_ps_weight; a.evw = d_event_weight; }
+  DeviceGuard g(p->par.device); if (!g.ok) return MG_ECUDA;
+  return cuda_rc(launch_me(p, a, (cudaStream_t)stream));
+}
+
+int mg_sigmakin_per_helicity(mg_process* p, const void* d_momenta, int64_t n, int64_t ld, void* d_me_hel, void* stream) {
+  int rc = check_soa(p, d_momenta, n, ld); if (rc != MG_OK || n == 0) return rc;
+  rc = check_soa(p, d_me_hel, n, ld); if (rc != MG_OK) return rc;
+  MeArgs a{d_momenta, n, ld, nullptr, nullptr, nullptr, d_me_hel, 0};
+  DeviceGuard g(p->par.device); if (!g.ok) return MG_ECUDA;
+  return cuda_rc(launch_me(p, a, (cudaStream_t)stream));
+}
+
+int mg_set_helicity_mask(mg_process* p, uint64_t mask) {
+  if (!p) return MG_EINVAL;
+  const uint64_t all = p->n_hel == 64 ? ~0ull : ((1ull << p->n_hel) - 1);
+  p->hel_mask = mask & all;
+  return MG_OK;
+}
+int mg_get_helicity_mask(const mg_process* p, uint64_t* out) {
+  if (!p || !out) return MG_EINVAL;
+  *out = p->hel_mask;
+  return MG_OK;
+}
+
+int mg_filter_helicities(mg_process* p, const void* d_momenta, int64_t probe_n, int64_t ld, uint64_t* h_out_mask, void* stream) {
+  if (!valid_handle(p) || probe_n <= 0 || probe_n > (1 << 20)) return MG_EINVAL;
+  int rc = check_soa(p, d_momenta, probe_n, ld); if (rc != MG_OK) return rc;
+  DeviceGuard g(p->par.device); if (!g.ok) return MG_ECUDA;
+  const size_t es = elem(p);
+  const int64_t pld = mg_padded_stride(probe_n);
+  void* d_hel = nullptr;
+  if (cudaMalloc(&d_hel, (size_t)pld * p->n_hel * es) != cudaSuccess) { cudaGetLastError(); return MG_ENOMEM; }
+  // the probe kernel indexes momenta with the caller's ld and the output with the same ld: use a
+  // compact copy of the probe momenta so that both strides are pld
+  void* d_mom = nullptr;
+  const int rows = 4 * p->n_ext;
+  if (cudaMalloc(&d_mom, (size_t)pld * rows * es) != cudaSuccess) { cudaGetLastError(); cudaFree(d_hel); return MG_ENOMEM; }
+  cudaStream_t s = (cudaStream_t)stream;
+  cudaError_t e = cudaMemcpy2DAsync(d_mom, (size_t)pld * es, d_momenta, (size_t)ld * es, (size_t)probe_n * es, rows, cudaMemcpyDeviceToDevice, s);
+  MeArgs a{d_mom, probe_n, pld, nullptr, nullptr, nullptr, d_hel, 0};
+  if (e == cudaSuccess) e = launch_me(p, a, s);
+  const size_t hb = (size_t)pld * p->n_hel * es;
+  void* h = malloc(hb);
+  if (!h) { cudaFree(d_hel); cudaFree(d_mom); return MG_ENOMEM; }
+  if (e == cudaSuccess) e = cudaMemcpyAsync(h, d_hel, hb, cudaMemcpyDeviceToHost, s);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(s);
+  cudaFree(d_hel); cudaFree(d_mom);
+  if (e != cudaSuccess) { cudaGetLastError(); free(h); return MG_ECUDA; }
+  // R16: h is good iff max over probe events of |M|^2_h / sum_h' |M|^2_h' > 1e-10.  (Selection on
+  // kernel outputs; the arithmetic of the path is all in the kernel.)
+  uint64_t mask = 0;
+  for (int64_t ev = 0; ev < probe_n; ++ev) {
+    double tot = 0;
+    for (int hh = 0; hh < p->n_hel; ++hh) tot += es == 8 ? ((double*)h)[hh * pld + ev] : (double)((float*)h)[hh * pld + ev];
+    if (!(tot > 0) || !isfinite(tot)) continue;
+    for (int hh = 0; hh < p->n_hel; ++hh) {
+      const double v = es == 8 ? ((double*)h)[hh * pld + ev] : (double)((float*)h)[hh * pld + ev];
+      if (v / tot > 1e-10) mask |= 1ull << hh;
+    }
+  }
+  free(h);
+  if (mask == 0) return MG_EPARAM;
+  p->hel_mask = mask;
+  if (h_out_mask) *h_out_mask = mask;
+  return MG_OK;
+}
+
+int mg_sigmakin_host(mg_process* p, const void* h_momenta, int64_t n, int64_t ld, void* h_me) {
+  if (!valid_handle(p) || n < 0) return MG_EINVAL;
+  if (n == 0) return MG_OK;
+  if (!h_momenta || !h_me || ld < n) return MG_EINVAL;
+  DeviceGuard g(p->par.device); if (!g.ok) return MG_ECUDA;
+  const size_t es = elem(p);
+  const int rows = 4 * p->n_ext;
+  const size_t mom_b = (size_t)ld * rows * es, me_b = (size_t)n * es;
+  const size_t me_off = (mom_b + 255) / 256 * 256;
+  int rc = ensure_scratch(p, me_off + me_b, 0); if (rc != MG_OK) return rc;
+  char* d = (char*)p->d_scratch;
+  cudaStream_t s = p->own_stream;
+  cudaError_t e = cudaMemcpyAsync(d, h_momenta, mom_b, cudaMemcpyHostToDevice, s);
+  if (e == cudaSuccess) e = cudaEventRecord(p->ev0, s);
+  MeArgs a{d, n, ld, d + me_off, nullptr, nullptr, nullptr, p->hel_mask};
+  if (e == cudaSuccess) e = launch_me(p, a, s);
+  if (e == cudaSuccess) e = cudaEventRecord(p->ev1, s);
+  if (e == cudaSuccess) e = cudaMemcpyAsync(h_me, d + me_off, me_b, cudaMemcpyDeviceToHost, s);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(s);
+  if (e != cudaSuccess) { cudaGetLastError(); return MG_ECUDA; }
+  float ms = 0; cudaEventElapsedTime(&ms, p->ev0, p->ev1); p->last_kernel_ms = ms;
+  return MG_OK;
+}
+
+int mg_run_host(mg_process* p, uint64_t seed, uint64_t first_event, int64_t n, int64_t ld, void* h_momenta, void* h_ps_weight, void* h_me) {
+  if (!valid_handle(p) || n < 0) return MG_EINVAL;
+  if (n == 0) return MG_OK;
+  if (!h_me || ld < n) return MG_EINVAL;
+  DeviceGuard g(p->par.device); if (!g.ok) return MG_ECUDA;
+  const size_t es = elem(p);
+  const int rows = 4 * p->n_ext;
+  const size_t mom_b = (size_t)ld * rows * es, vec_b = ((size_t)n * es + 255) / 256 * 256;
+  const size_t mom_off = 0, w_off = (mom_b + 255) / 256 * 256, me_off = w_off + vec_b;
+  int rc = ensure_scratch(p, me_off + vec_b, 0); if (rc != MG_OK) return rc;
+  char* d = (char*)p->d_scratch;
+  cudaStream_t s = p->own_stream;
+  cudaError_t e = launch_generate(p, seed, first_event, n, ld, d + mom_off, d + w_off, s);
+  if (e == cudaSuccess) e = cudaEventRecord(p->ev0, s);
+  MeArgs a{d + mom_off, n, ld, d + me_off, nullptr, nullptr, nullptr, p->hel_mask};
+  if (e == cudaSuccess) e = launch_me(p, a, s);
+  if (e == cudaSuccess) e = cudaEventRecord(p->ev1, s);
+  if (e == cudaSuccess && h_momenta) e = cudaMemcpyAsync(h_momenta, d + mom_off, mom_b, cudaMemcpyDeviceToHost, s);
+  if (e == cudaSuccess && h_ps_weight) e = cudaMemcpyAsync(h_ps_weight, d + w_off, (size_t)n * es, cudaMemcpyDeviceToHost, s);
+  if (e == cudaSuccess) e = cudaMemcpyAsync(h_me, d + me_off, (size_t)n * es, cudaMemcpyDeviceToHost, s);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(s);
+  if (e != cudaSuccess) { cudaGetLastError(); return MG_ECUDA; }
+  float ms = 0; cudaEventElapsedTime(&ms, p->ev0, p->ev1); p->last_kernel_ms = ms;
+  return MG_OK;
+}
+
+int64_t mg_flops_per_event(const mg_process* p, int stage) {
+  if (!p) return MG_EINVAL;
+  if (stage == MG_STAGE_SIGMAKIN) {
+    const int good = __builtin_popcountll(p->hel_mask);
+    return me_flops_per_event_fixed(p->par.process) + (int64_t)good * me_flops_per_helicity(p->par.process);
+  }
+  return 0;  // the RNG and RAMBO stages are HBM-bound; their roofline is bytes (mg_bytes_per_event)
+}
+
+int64_t mg_bytes_per_event(const mg_process* p, int stage) {
+  if (!p) return MG_EINVAL;
+  const int64_t es = (int64_t)elem(p);
+  switch (stage) {
+    case MG_STAGE_RNG: return es * 4 * p->n_final;                                         // write uniforms
+    case MG_STAGE_RAMBO: return es * (4 * p->n_final + 4 * p->n_ext + 1);                  // read uniforms, write momenta + weight
+    case MG_STAGE_SIGMAKIN: return es * (4 * p->n_ext + 1);                                // read momenta, write ME
+    case MG_STAGE_GENERATE: return es * (4 * p->n_ext + 1);                                // write momenta + weight
+  }
+  return MG_EINVAL;
+}
+
+double mg_last_kernel_ms(const mg_process* p) { return p ? p->last_kernel_ms : 0.0; }
+
+const char* mg_strerror(int code) {
+  switch (code) {
+    case MG_OK: return "ok";
+    case MG_EINVAL: return "invalid argument (null/misaligned pointer, bad size, stride or id)";
+    case MG_EPARAM: return "unphysical parameters";
+    case MG_ECUDA: return "CUDA error or no sm_100 device";
+    case MG_ENOMEM: return "out of memory";
+  }
+  return "unknown error";
+}
+const char* mg_version(void) { return "mg-b200 0.1 (sm_100a)"; }
+
+}  // extern "C"
