@@ -142,6 +142,11 @@ int64_t mg_bytes_per_event(const mg_process* p, int stage);
  * the library's stream (0 if none). */
 double mg_last_kernel_ms(const mg_process* p);
 
+/* Measured FMA throughput of the plain FP64 / FP32 ALUs of `device` in TFLOP/s (FMA = 2): a
+ * register-only chain microbenchmark (the denominator of the "alu" roofline).
+ * Synchronous, takes ~0.1 s. */
+int mg_measure_alu_peak(int precision, int device, double* h_tflops_out);
+
 const char* mg_strerror(int code);
 const char* mg_version(void);
 

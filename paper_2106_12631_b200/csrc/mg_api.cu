@@ -338,6 +338,14 @@ int64_t mg_bytes_per_event(const mg_process* p, int stage) {
   return MG_EINVAL;
 }
 
+int mg_measure_alu_peak(int precision, int device, double* h_tflops_out) {
+  if (!h_tflops_out || device < 0 || (precision != MG_FP64 && precision != MG_FP32)) return MG_EINVAL;
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || device >= ndev) { cudaGetLastError(); return MG_ECUDA; }
+  DeviceGuard g(device); if (!g.ok) return MG_ECUDA;
+  return cuda_rc(measure_alu_peak(precision, device, h_tflops_out));
+}
+
 double mg_last_kernel_ms(const mg_process* p) { return p ? p->last_kernel_ms : 0.0; }
 
 const char* mg_strerror(int code) {

@@ -311,12 +311,12 @@ class Generator:
         ng = self.ng
         nf = len(self.flows)
         strings = np.zeros((nf,) + (8,) * ng + (3, 3), dtype=complex)
+        letters = "abcd"
         for f, perm in enumerate(self.flows):
-            for a in itertools.product(range(8), repeat=ng):
-                M = np.eye(3, dtype=complex)
-                for pos in range(ng):
-                    M = M @ T[a[perm[pos]]]
-                strings[(f,) + a] = M
+            # (T^{a_perm[0]} T^{a_perm[1]} ...)_{ij} for all colour assignments at once
+            spec = ",".join(letters[perm[pos]] + "ijklm"[pos] + "ijklm"[pos + 1] for pos in range(ng))
+            spec += "->" + letters[:ng] + "i" + "ijklm"[ng]
+            strings[f] = np.einsum(spec, *([T] * ng))
         flat = strings.reshape(nf, -1)
         C = (flat @ flat.conj().T).real
         den = {2: 3, 3: 9, 4: 54}[ng]
@@ -391,13 +391,13 @@ class Emitter:
         w("}  // namespace mg")
         return "\n".join(self.lines) + "\n", num, den
 
-    def _mom_lines(self, ev="ev."):
+    def _mom_lines(self, ev="ev.p", T="T"):
         """local momentum definitions used by both finish() and helicity()"""
         g = self.g
         out = []
         for gi in range(g.ng):
             ip = g.gl_particle[gi]
-            out.append("    const Mom<T> K%d = %s%sp[%d];" % (gi, "" if gi < 2 else "-", ev, ip))
+            out.append("    const Mom<T> K%d = %s%s[%d];" % (gi, "" if gi < 2 else "-", ev, ip))
         for S in self.gsets:
             parts = sorted(S)
             # build from the largest already-defined subset
@@ -406,7 +406,7 @@ class Emitter:
             else:
                 sub = frozenset(parts[:-1])
                 out.append("    const Mom<T> %s = %s + K%d;" % (self.kname(S), self.kname(sub), parts[-1]))
-        out.append("    const Mom<T> pt = %sp[2], ptb = %sp[3];" % (ev, ev))
+        out.append("    const Mom<T> pt = %s[2], ptb = %s[3];" % (ev, ev))
         for key in self.qkeys:
             side, S = key
             kn = self.kname(S) if len(S) > 1 else "K%d" % sorted(S)[0]
@@ -414,24 +414,28 @@ class Emitter:
                 out.append("    const Mom<T> %s = pt - %s;" % (self.qname(key), kn))
             else:
                 out.append("    const Mom<T> %s = %s - ptb;" % (self.qname(key), kn))
-        return out
+        return [l.replace("Mom<T>", "Mom<%s>" % T) for l in out]
 
     def _emit_momenta_fn(self):
         pass
 
     def _emit_finish(self):
         w = self.w
-        w("  // helicity-independent part: inverse propagator denominators")
+        w("  // helicity-independent part: inverse propagator denominators.  Always evaluated in double")
+        w("  // (also for T = float): k_i.k_j cancels like 1/theta^2 for collinear pairs, and this is once per")
+        w("  // event, not once per helicity (DESIGN.md R19 / mixed precision).")
         w("  template <class T> static MG_HD void finish(Event<T>& ev, const Consts& k) {")
-        for l in self._mom_lines():
+        w("    Mom<double> pd[NPAR];")
+        w("    for (int i = 0; i < NPAR; ++i) for (int mu = 0; mu < 4; ++mu) pd[i].v[mu] = (double)ev.p[i].v[mu];")
+        for l in self._mom_lines(ev="pd", T="double"):
             w(l)
-        w("    const T mt2 = (T)k.mt * (T)k.mt;")
+        w("    const double mt2 = k.mt * k.mt;")
         for S in self.gsets:
-            w("    ev.ik[%d] = (T)1 / mdot(%s, %s);" % (self.ik_index[S], self.kname(S), self.kname(S)))
+            w("    ev.ik[%d] = (T)(1.0 / mdot(%s, %s));" % (self.ik_index[S], self.kname(S), self.kname(S)))
             self.flops_fixed += 8 + 4 * (len(S) - 1)
-        w("    { const Mom<T> Kf = pt + ptb; ev.ik[%d] = (T)1 / mdot(Kf, Kf); }" % self.ik_full)
+        w("    { const Mom<double> Kf = pt + ptb; ev.ik[%d] = (T)(1.0 / mdot(Kf, Kf)); }" % self.ik_full)
         for key in self.qkeys:
-            w("    ev.iq[%d] = (T)1 / (mdot(%s, %s) - mt2);" % (self.iq_index[key], self.qname(key), self.qname(key)))
+            w("    ev.iq[%d] = (T)(1.0 / (mdot(%s, %s) - mt2));" % (self.iq_index[key], self.qname(key), self.qname(key)))
             self.flops_fixed += 13
         w("  }")
         w("")
