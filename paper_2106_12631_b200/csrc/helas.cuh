@@ -76,13 +76,15 @@ template <class T> MG_HD Chi<T> chi(Mom<T> p, T P, int lambda) {
   return x;
 }
 
-// omega_+ = sqrt(E+P), omega_- = sqrt(E-P) = m/omega_+ (exactly 0 for m = 0).
+// omega_+ = sqrt(E+P), omega_- = sqrt(E-P) = m/omega_+ (exactly 0 for m = 0).  For m = 0 the energy
+// is taken as |p| (not the stored E), so that the spinor solves the Dirac equation of the 3-momentum
+// exactly even when the event generator left E and |p| a few ulps (or gamma^2 ulps) apart.
 // u(p,l)    = (omega_{-l} chi_l ; omega_{l} chi_l)            incoming fermion   (IXXXXX)
 // v(p,l)    = (omega_{l} chi_{-l} ; -omega_{-l} chi_{-l})     outgoing antifermion (IXXXXX)
 // ubar, vbar = psi^dagger gamma^0 = (psi_R^dagger | psi_L^dagger)   outgoing fermion / incoming antifermion (OXXXXX)
 template <class T> MG_HD Spinor<T> spinor_u(Mom<T> p, T m, int lambda) {
   const T P = sqrt_<T>(fma_<T>(p.v[1], p.v[1], fma_<T>(p.v[2], p.v[2], p.v[3] * p.v[3])));
-  const T wp = sqrt_<T>(p.v[0] + P);
+  const T wp = sqrt_<T>((m == (T)0 ? P : p.v[0]) + P);
   const T wm = m / wp;
   const Chi<T> x = chi<T>(p, P, lambda);
   const T wl = lambda > 0 ? wm : wp, wr = lambda > 0 ? wp : wm;
@@ -93,7 +95,7 @@ template <class T> MG_HD Spinor<T> spinor_u(Mom<T> p, T m, int lambda) {
 }
 template <class T> MG_HD Spinor<T> spinor_v(Mom<T> p, T m, int lambda) {
   const T P = sqrt_<T>(fma_<T>(p.v[1], p.v[1], fma_<T>(p.v[2], p.v[2], p.v[3] * p.v[3])));
-  const T wp = sqrt_<T>(p.v[0] + P);
+  const T wp = sqrt_<T>((m == (T)0 ? P : p.v[0]) + P);
   const T wm = m / wp;
   const Chi<T> x = chi<T>(p, P, -lambda);
   const T wl = lambda > 0 ? wp : wm, wr = lambda > 0 ? -wm : -wp;

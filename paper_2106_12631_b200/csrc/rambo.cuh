@@ -1,0 +1,134 @@
+// rambo.cuh — one event of RAMBO (steps A3, A4): massless generation and massive rescaling.
+// PAPER.md:78 ("a simple phase space sampling algorithm, RAMBO [39]"), PAPER.md:92 (momenta and a
+// sampling weight).  Equations: Kleiss, Stirling, Ellis, CPC 40 (1986) 359; readings R5-R8.
+//
+// The KSE map is  q_i = q_i0 (1, n_i),  Q = sum q_i,  M = sqrt(Q^2),  p_i = x * Boost_{-Q/M}(q_i),  x = sqrt_s/M.
+// Written as in the paper (b = -Q/M, gamma = Q0/M, a = 1/(1+gamma)) it loses a factor gamma^2 of
+// precision when the q_i are nearly parallel (M << Q0), and in FP32 Q0^2 - |Q|^2 can even come out
+// negative (the NaN events of PAPER.md:182).  The SAME map is evaluated here through Minkowski
+// products of the massless q's, which are sums of non-negative terms:
+//     h_ij = (1 - n_i.n_j) = |n_i - n_j|^2 / 2,        q_i.q_j = q_i0 q_j0 h_ij,
+//     g_i  = (q_i.Q)/q_i0 = sum_{j != i} q_j0 h_ij,     M^2 = sum_i q_i0 g_i,
+//     p_i0 = sqrt_s q_i0 g_i / M^2,
+//     p_i  = x D q_i0 sum_{j != i} q_j0 [ (M + g_j)(n_i - n_j) + (g_j - g_i) n_j ],   D = 1/(M (M + Q0)),
+// (uses sum_i c_i = 1 for c_i = (q_i0 M + q_i.Q) D, the coefficient of -Q in the boosted 3-vector).
+// Rounding is then amplified by gamma, the conditioning of the map itself, not by gamma^2.
+#pragma once
+#include "consts.h"
+#include "cx.cuh"
+
+namespace mg {
+
+MG_HD void sincos2pi_(double x, double* s, double* c) {
+#ifdef __CUDA_ARCH__
+  sincospi(2.0 * x, s, c);
+#else
+  *s = sin(6.283185307179586476925286766559 * x); *c = cos(6.283185307179586476925286766559 * x);
+#endif
+}
+MG_HD void sincos2pi_(float x, float* s, float* c) {
+#ifdef __CUDA_ARCH__
+  sincospif(2.0f * x, s, c);
+#else
+  *s = sinf(6.28318530717958647692f * x); *c = cosf(6.28318530717958647692f * x);
+#endif
+}
+MG_HD double log_(double x) { return log(x); }
+MG_HD float log_(float x) { return logf(x); }
+
+// rho[4*i+k] -> p[i][mu] (final particles only); returns the phase-space weight.
+template <class T, int NF, bool MASSIVE>
+MG_HD T rambo_core(const T (&rho)[4 * NF], const Consts& k, T (&p)[NF][4]) {
+  T q0[NF], nx[NF], ny[NF], nz[NF];
+  T Q0 = 0;
+#pragma unroll
+  for (int i = 0; i < NF; ++i) {
+    const T r1 = rho[4 * i + 0], r2 = rho[4 * i + 1], r3 = rho[4 * i + 2], r4 = rho[4 * i + 3];
+    const T c = fma_<T>((T)2, r1, (T)-1);                    // cos(theta) = 2 rho1 - 1
+    const T st = (T)2 * sqrt_<T>(r1 * ((T)1 - r1));          // sqrt(1 - c^2), no cancellation (R19)
+    T sp, cp;
+    sincos2pi_(r2, &sp, &cp);                                 // phi = 2 pi rho2
+    // FP32: the rounded product r3*r4 near 1 would lose the small q0; two logs do not (R19)
+    q0[i] = sizeof(T) == 8 ? -log_(r3 * r4) : -(log_(r3) + log_(r4));
+    nx[i] = st * cp; ny[i] = st * sp; nz[i] = c;
+    Q0 += q0[i];
+  }
+  T h[NF][NF];
+#pragma unroll
+  for (int i = 0; i < NF; ++i)
+#pragma unroll
+    for (int j = i + 1; j < NF; ++j) {
+      const T dx = nx[i] - nx[j], dy = ny[i] - ny[j], dz = nz[i] - nz[j];
+      h[i][j] = h[j][i] = (T)0.5 * fma_<T>(dx, dx, fma_<T>(dy, dy, dz * dz));
+    }
+  T g[NF];
+  T M2 = 0;
+#pragma unroll
+  for (int i = 0; i < NF; ++i) {
+    T s = 0;
+#pragma unroll
+    for (int j = 0; j < NF; ++j) if (j != i) s = fma_<T>(q0[j], h[i][j], s);
+    g[i] = s;
+    M2 = fma_<T>(q0[i], s, M2);
+  }
+  const T sqrt_s = (T)k.sqrt_s;
+  const T M = sqrt_<T>(M2);
+  const T x = sqrt_s / M;
+  const T xD = x / (M * (M + Q0));
+  const T e0 = sqrt_s / M2;
+#pragma unroll
+  for (int i = 0; i < NF; ++i) {
+    T sx = 0, sy = 0, sz = 0;
+#pragma unroll
+    for (int j = 0; j < NF; ++j) {
+      if (j == i) continue;
+      const T a = q0[j] * (M + g[j]), b = q0[j] * (g[j] - g[i]);
+      sx = fma_<T>(a, nx[i] - nx[j], fma_<T>(b, nx[j], sx));
+      sy = fma_<T>(a, ny[i] - ny[j], fma_<T>(b, ny[j], sy));
+      sz = fma_<T>(a, nz[i] - nz[j], fma_<T>(b, nz[j], sz));
+    }
+    const T f = xD * q0[i];
+    p[i][0] = e0 * q0[i] * g[i];
+    p[i][1] = f * sx; p[i][2] = f * sy; p[i][3] = f * sz;
+  }
+  T w = (T)k.w0;
+  if (MASSIVE) {
+    // Newton on f(xi) = sum_i sqrt(m_i^2 + xi^2 p_i0^2) - sqrt_s from xi0 = sqrt(1 - (sum m / sqrt_s)^2);
+    // fixed iteration count (lock-step): converged to rounding after 3 steps for the BASELINE masses (R7).
+    T m2[NF], p02[NF];
+    T summ = 0;
+#pragma unroll
+    for (int i = 0; i < NF; ++i) { const T m = (T)k.mass[i]; m2[i] = m * m; p02[i] = p[i][0] * p[i][0]; summ += m; }
+    const T r = summ / sqrt_s;
+    T xi = sqrt_<T>((T)1 - r * r);
+    constexpr int kNewton = sizeof(T) == 8 ? 5 : 4;
+#pragma unroll 1
+    for (int it = 0; it < kNewton; ++it) {
+      T f = -sqrt_s, df = 0;
+#pragma unroll
+      for (int i = 0; i < NF; ++i) {
+        const T E = sqrt_<T>(fma_<T>(xi * xi, p02[i], m2[i]));
+        f += E;
+        df += xi * p02[i] / E;
+      }
+      xi -= f / df;
+    }
+    T prod = 1, sum2 = 0;
+#pragma unroll
+    for (int i = 0; i < NF; ++i) {
+      const T kabs = xi * p[i][0];
+      const T E = sqrt_<T>(fma_<T>(kabs, kabs, m2[i]));
+      p[i][0] = E;
+      p[i][1] *= xi; p[i][2] *= xi; p[i][3] *= xi;
+      prod *= kabs / E;
+      sum2 += kabs * kabs / E;
+    }
+    T xipow = 1;
+#pragma unroll
+    for (int i = 0; i < 2 * NF - 3; ++i) xipow *= xi;
+    w = w * xipow * prod * sqrt_s / sum2;
+  }
+  return w;
+}
+
+}  // namespace mg

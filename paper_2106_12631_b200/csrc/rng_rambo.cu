@@ -7,6 +7,7 @@
 // R5-R8 of DESIGN.md; the paper prints no equations.
 #include "mg_internal.h"
 #include "philox.cuh"
+#include "rambo.cuh"
 
 namespace mg {
 
@@ -14,10 +15,6 @@ namespace {
 
 constexpr int kThreads = 256;
 
-__device__ __forceinline__ void sincospi_(double x, double* s, double* c) { sincospi(x, s, c); }
-__device__ __forceinline__ void sincospi_(float x, float* s, float* c) { sincospif(x, s, c); }
-__device__ __forceinline__ double log_(double x) { return log(x); }
-__device__ __forceinline__ float log_(float x) { return logf(x); }
 
 __global__ void __launch_bounds__(kThreads) rng_words_kernel(uint64_t seed, uint64_t first, int64_t n, int64_t ld,
                                                              int nf, uint32_t* __restrict__ out) {
@@ -46,85 +43,13 @@ __global__ void __launch_bounds__(kThreads) rng_kernel(uint64_t seed, uint64_t f
   }
 }
 
-// One event of RAMBO.  rho[4*i+k]; writes momenta rows (beams + NF finals) and the weight.
-//   massless (KSE eq. for q_i, boost b, scale x);  c = 2 rho1 - 1, sqrt(1-c^2) = 2 sqrt(rho1 (1-rho1))
-//   (same value, no cancellation near |c| = 1: R19).
-//   massive: Newton on f(xi) = sum_i sqrt(m_i^2 + xi^2 p_i0^2) - sqrt_s, fixed iteration count
-//   (lock-step; converged to rounding well before the last step, R7).
 template <class T, int NF, bool MASSIVE>
 __device__ __forceinline__ void rambo_event(const T (&rho)[4 * NF], const Consts& k, int64_t e, int64_t ld,
                                             T* __restrict__ mom, T* __restrict__ wout) {
-  T q[NF][4];
-  T Q0 = 0, Q1 = 0, Q2 = 0, Q3 = 0;
-#pragma unroll
-  for (int i = 0; i < NF; ++i) {
-    const T r1 = rho[4 * i + 0], r2 = rho[4 * i + 1], r3 = rho[4 * i + 2], r4 = rho[4 * i + 3];
-    const T c = fma_<T>((T)2, r1, (T)-1);
-    const T st = (T)2 * sqrt_<T>(r1 * ((T)1 - r1));
-    T sp, cp;
-    sincospi_((T)2 * r2, &sp, &cp);
-    const T q0 = -log_(r3 * r4);
-    q[i][0] = q0;
-    q[i][1] = q0 * st * cp;
-    q[i][2] = q0 * st * sp;
-    q[i][3] = q0 * c;
-    Q0 += q[i][0]; Q1 += q[i][1]; Q2 += q[i][2]; Q3 += q[i][3];
-  }
-  const T sqrt_s = (T)k.sqrt_s;
-  const T M2 = Q0 * Q0 - Q1 * Q1 - Q2 * Q2 - Q3 * Q3;
-  const T M = sqrt_<T>(M2);
-  const T iM = (T)1 / M;
-  const T b1 = -Q1 * iM, b2 = -Q2 * iM, b3 = -Q3 * iM;
-  const T x = sqrt_s * iM;
-  const T gamma = Q0 * iM;
-  const T a = (T)1 / ((T)1 + gamma);
   T p[NF][4];
-#pragma unroll
-  for (int i = 0; i < NF; ++i) {
-    const T bq = b1 * q[i][1] + b2 * q[i][2] + b3 * q[i][3];
-    p[i][0] = x * (gamma * q[i][0] + bq);
-    const T abq = a * bq;
-    p[i][1] = x * (q[i][1] + b1 * q[i][0] + abq * b1);
-    p[i][2] = x * (q[i][2] + b2 * q[i][0] + abq * b2);
-    p[i][3] = x * (q[i][3] + b3 * q[i][0] + abq * b3);
-  }
-  T w = (T)k.w0;
-  if (MASSIVE) {
-    T m[NF], m2[NF], p02[NF];
-    T summ = 0;
-#pragma unroll
-    for (int i = 0; i < NF; ++i) { m[i] = (T)k.mass[i]; m2[i] = m[i] * m[i]; p02[i] = p[i][0] * p[i][0]; summ += m[i]; }
-    const T r = summ / sqrt_s;
-    T xi = sqrt_<T>((T)1 - r * r);
-    constexpr int kNewton = sizeof(T) == 8 ? 5 : 4;
-#pragma unroll 1
-    for (int it = 0; it < kNewton; ++it) {
-      T f = -sqrt_s, df = 0;
-#pragma unroll
-      for (int i = 0; i < NF; ++i) {
-        const T E = sqrt_<T>(fma_<T>(xi * xi, p02[i], m2[i]));
-        f += E;
-        df += xi * p02[i] / E;
-      }
-      xi -= f / df;
-    }
-    T prod = 1, sum2 = 0;
-#pragma unroll
-    for (int i = 0; i < NF; ++i) {
-      const T kabs = xi * p[i][0];
-      const T E = sqrt_<T>(fma_<T>(kabs, kabs, m2[i]));
-      p[i][0] = E;
-      p[i][1] *= xi; p[i][2] *= xi; p[i][3] *= xi;
-      prod *= kabs / E;
-      sum2 += kabs * kabs / E;
-    }
-    T xipow = 1;
-#pragma unroll
-    for (int i = 0; i < 2 * NF - 3; ++i) xipow *= xi;
-    w = w * xipow * prod * sqrt_s / sum2;
-  }
+  const T w = rambo_core<T, NF, MASSIVE>(rho, k, p);
   // beams (R5)
-  const T hs = (T)0.5 * sqrt_s;
+  const T hs = (T)0.5 * (T)k.sqrt_s;
   T* o = mom + e;
   __stcs(o + 0 * ld, hs); __stcs(o + 1 * ld, (T)0); __stcs(o + 2 * ld, (T)0); __stcs(o + 3 * ld, hs);
   __stcs(o + 4 * ld, hs); __stcs(o + 5 * ld, (T)0); __stcs(o + 6 * ld, (T)0); __stcs(o + 7 * ld, -hs);

@@ -5,8 +5,10 @@ Tolerances (north_star; DESIGN.md "Tolerances"):
   RNG words and uniforms          bit-exact
   RAMBO  FP64                     |dp| <= 1e-12 sqrt_s per component, |dW|/W <= 1e-12   (same uniforms)
          FP32                     1e-5 sqrt_s, 1e-5
-         ill-conditioned tail: the KSE boost amplifies rounding by gamma^2 = (Q0/M)^2; such events are
-         counted, printed and held to 1e-12 * gamma^2 (never silently).
+         The reference is the oracle run in LONG DOUBLE: the plain KSE boost in double loses a factor
+         gamma^2 = (Q0/M)^2 of precision for nearly parallel q_i (3e-11 sqrt_s seen), more than the
+         tolerance; the CUDA path evaluates the same map in a form that loses only gamma (rambo.cuh).
+         FP32: events with gamma > 32 are held to 1e-5 * gamma/32, counted and printed.
   ME     FP64                     |ME_gpu/ME_oracle - 1| <= 1e-12 per event (oracle fed the GPU's momenta)
          FP32                     <= 1e-4 per event and <= 1e-6 on the batch mean
          ill-conditioned tail (FP64): an event may exceed 1e-12 only if the double oracle itself is more
@@ -77,7 +79,7 @@ def _rambo_compare(mg, process, prec, n, seed):
     rnd = P.rng(seed, 0, n)
     mom, w = P.rambo(rnd, n)
     rho = soa_to_aos(_np(rnd, n).astype(np.float64), P.n_final)
-    mom_o, w_o, _ = oracle.rambo(rho, oracle.masses(process), SQRT_S)
+    mom_o, w_o, _ = oracle.rambo(rho, oracle.masses(process), SQRT_S, long_double=True)
     mom_g = soa_to_aos(_np(mom, n).astype(np.float64), P.n_external)
     w_g = w[:n].cpu().numpy().astype(np.float64)
     # conditioning of the KSE boost: gamma = Q0 / M of the massless q's
@@ -86,42 +88,50 @@ def _rambo_compare(mg, process, prec, n, seed):
     phi = 2 * np.pi * rho[:, :, 1]
     q0 = -np.log(rho[:, :, 2] * rho[:, :, 3])
     Q = np.stack([q0, q0 * st * np.cos(phi), q0 * st * np.sin(phi), q0 * c], -1).sum(1)
-    gamma2 = Q[:, 0] ** 2 / (Q[:, 0] ** 2 - (Q[:, 1:] ** 2).sum(-1))
-    return mom_g, w_g, mom_o, w_o, gamma2
+    gamma = Q[:, 0] / np.sqrt(Q[:, 0] ** 2 - (Q[:, 1:] ** 2).sum(-1))
+    return mom_g, w_g, mom_o, w_o, gamma
 
 
 @pytest.mark.parametrize("process", PROCS)
 def test_rambo_fp64(mg, process):
-    n = 16384 + 37     # several blocks and a ragged tail
-    mom_g, w_g, mom_o, w_o, g2 = _rambo_compare(mg, process, 0, n, 42)
+    n = 65536 + 37     # several hundred blocks and a ragged tail
+    mom_g, w_g, mom_o, w_o, gamma = _rambo_compare(mg, process, 0, n, 42)
     dp = np.abs(mom_g - mom_o).max(axis=(1, 2)) / SQRT_S
     dw = np.abs(w_g / w_o - 1)
-    tol = 1e-12 * np.maximum(1.0, g2 / 16.0)
-    tail = (dp > 1e-12) | (dw > 1e-12)
-    print("rambo fp64 process %d: max dp/sqrt_s %.2e, max dW/W %.2e, ill-conditioned tail %d of %d (max gamma^2 %.1e)"
-          % (process, dp.max(), dw.max(), tail.sum(), n, g2.max()))
-    assert (dp <= tol).all() and (dw <= tol).all()
-    assert tail.sum() <= n // 1000
-    # invariants on the GPU output itself
+    print("rambo fp64 process %d: max dp/sqrt_s %.2e, max dW/W %.2e (max gamma %.1e)" % (process, dp.max(), dw.max(), gamma.max()))
+    assert dp.max() <= 1e-12 and dw.max() <= 1e-12
+    # invariants on the GPU output itself: momentum conservation and on-shellness
     tot = mom_g[:, 2:].sum(1)
-    assert np.abs(tot - np.array([SQRT_S, 0, 0, 0])).max() < 1e-9 * np.sqrt(g2.max())
+    assert np.abs(tot - np.array([SQRT_S, 0, 0, 0])).max() < 1e-12 * SQRT_S
     m2 = mom_g[..., 0] ** 2 - (mom_g[..., 1:] ** 2).sum(-1)
     masses = np.concatenate([[0, 0], oracle.masses(process)])
-    assert np.abs(m2 - masses**2).max() < 1e-9 * SQRT_S**2 * max(1.0, g2.max() / 1e4)
+    assert np.abs(m2 - masses**2).max() < 1e-12 * SQRT_S**2
     assert np.array_equal(mom_g[:, 0], np.tile([750.0, 0, 0, 750.0], (n, 1)))
     assert np.array_equal(mom_g[:, 1], np.tile([750.0, 0, 0, -750.0], (n, 1)))
 
 
 @pytest.mark.parametrize("process", PROCS)
 def test_rambo_fp32(mg, process):
-    n = 8192 + 5
-    mom_g, w_g, mom_o, w_o, g2 = _rambo_compare(mg, process, 1, n, 7)
+    n = 65536 + 5
+    mom_g, w_g, mom_o, w_o, gamma = _rambo_compare(mg, process, 1, n, 7)
     dp = np.abs(mom_g - mom_o).max(axis=(1, 2)) / SQRT_S
     dw = np.abs(w_g / w_o - 1)
-    tol = 1e-5 * np.maximum(1.0, g2 / 16.0)
-    print("rambo fp32 process %d: max dp/sqrt_s %.2e, max dW/W %.2e" % (process, dp.max(), dw.max()))
+    tol = 1e-5 * np.maximum(1.0, gamma / 32.0)
+    print("rambo fp32 process %d: max dp/sqrt_s %.2e, max dW/W %.2e, events with gamma > 32: %d of %d"
+          % (process, dp.max(), dw.max(), (gamma > 32).sum(), n))
     assert np.isfinite(mom_g).all() and np.isfinite(w_g).all()
     assert (dp <= tol).all() and (dw <= tol).all()
+    assert (gamma > 32).sum() <= n // 500
+
+
+def test_rambo_fp32_has_no_nan_on_a_large_batch(mg):
+    # about one e+e- -> mu+mu- event in 10^6 gave NaN in FP32; here none may (R19)
+    n = 1 << 24
+    P = mg.Process(0, 1)
+    mom, w = P.generate(7, 0, n)
+    me = P.sigmakin(mom, n)
+    assert bool(torch.isfinite(mom[:, :n]).all()) and bool(torch.isfinite(w[:n]).all())
+    assert bool(torch.isfinite(me[:n]).all()) and bool((me[:n] > 0).all())
 
 
 @pytest.mark.parametrize("prec", [0, 1])
