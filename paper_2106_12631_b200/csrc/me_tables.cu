@@ -1,6 +1,7 @@
 // me_tables.cu — generated tables (flop tallies, colour matrices) behind mg_flops_per_event / mg_colour_matrix.
 #include "mg_internal.h"
 #include "gen_tables.cuh"
+#include "gen_rc_tables.cuh"
 
 namespace mg {
 
@@ -27,6 +28,14 @@ int64_t me_flops_per_event_fixed(int process) {
     case MG_GGTTGG: return kFlopsFixed_4;
   }
   return 0;
+}
+// processes evaluated by the helicity-recycling kernel (recycle.cuh): the tally of everything that kernel
+// executes per event (all helicity variants of every shared wavefunction); -1: per-helicity tally applies
+int64_t me_flops_per_event_recycle(int process) {
+  switch (process) {
+    case MG_GGTTGG: return kFlopsRecycle_4;
+  }
+  return -1;
 }
 const int* me_colour_numerators(int process, int* den) {
   switch (process) {

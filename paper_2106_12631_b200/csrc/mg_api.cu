@@ -320,6 +320,8 @@ int mg_run_host(mg_process* p, uint64_t seed, uint64_t first_event, int64_t n, i
 int64_t mg_flops_per_event(const mg_process* p, int stage) {
   if (!p) return MG_EINVAL;
   if (stage == MG_STAGE_SIGMAKIN) {
+    const int64_t rc = me_flops_per_event_recycle(p->par.process);
+    if (rc >= 0) return rc;
     const int good = __builtin_popcountll(p->hel_mask);
     return me_flops_per_event_fixed(p->par.process) + (int64_t)good * me_flops_per_helicity(p->par.process);
   }

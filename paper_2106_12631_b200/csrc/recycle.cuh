@@ -1,0 +1,287 @@
+// recycle.cuh — sigmaKin with HELICITY RECYCLING in shared memory: the sm_100a mapping
+// of steps A5-A11 for the processes whose live set does not fit one thread's registers.
+//
+// PAPER.md:136-138 names the register pressure of the one-thread-per-event sigmaKin kernel and lists the
+// remedies: shared memory for the wavefunctions, smaller kernels, or "different threads process different
+// helicities of the same event".  This kernel combines the first and the last:
+//   * a CTA works on E events; thread (e, h) owns helicity combination h of event e;
+//   * a wavefunction depends only on the helicities of the external legs it contains.  Each distinct
+//     (wavefunction, helicity variant) is a TASK computed once per event by one thread and stored in
+//     shared memory (wavefunctions shared between diagrams -> also shared between helicities);
+//   * a diagram psibar.Vslash.psi is closed as an inner product of a stored row spinor with a stored
+//     column spinor (the half product Vslash.psi or psibar.Vslash is itself a task); diagrams made of gluon
+//     trees only are closed as  J(all gluons) . G(t t~ current);
+//   * what stays per helicity: the inner products, the +-1 colour-flow sums (jamps in registers), the colour
+//     quadratic form, and the reduction over the helicity lanes.
+// The task tables (which node, which operands, which momentum, which propagator) and the unrolled
+// per-helicity code are written by gen/recycle.py; this header holds the generic task routines and the kernel.
+//
+// Shared-memory entry layout: entry i of event e holds 4 complex numbers (a Vec4 or a Spinor l0,l1,r0,r1),
+// stored component-major  ent[e][k][i], k = 0..3, one 16-byte (FP64) / 8-byte (FP32) word each.  A node with
+// nbits helicity bits owns 2^nbits consecutive entries (variant index = its helicity bits, compacted in
+// particle order).  Lanes of a warp are helicities of one event, so one request touches <= 2^nbits
+// consecutive words: broadcast, conflict-free.
+#pragma once
+#include "me_common.cuh"
+
+namespace mg {
+namespace rc {
+
+enum Kind { K_POLVEC = 0, K_UBAR = 1, K_VSP = 2, K_VCUR = 3, K_ROWPROP = 4, K_COLPROP = 5, K_FFCUR = 6, K_SLASHCOL = 7, K_SLASHROW = 8 };
+
+struct Op { short slot; short mask; };   // operand: first entry, and which of the consumer's variant bits select its variant
+struct NodeDesc {
+  short out;        // first entry of the result
+  short prop;       // index into the inverse-propagator table, -1: none
+  short mom;        // momentum-table index (line momentum of a propagator; particle momentum of an external)
+  short aux;        // K_POLVEC: 1 = outgoing;  K_VCUR: first term
+  short nterm;      // K_VCUR: number of terms
+  Op op[2];
+};
+struct TermDesc {   // one term of a gluon current: type 0: V3(A,kA,B,kB);  1..3: four-gluon structure `type`(A,B,C)
+  short type, sign;
+  short momA, momB;
+  Op op[3];
+};
+struct MomDef { signed char c[6]; signed char propkind; signed char pad; };   // momentum = sum_i c[i] p_i ; 0 none, 1: 1/q^2, 2: 1/(q^2-mt^2)
+
+template <class T> struct V2;
+template <> struct V2<double> { typedef double2 type; };
+template <> struct V2<float> { typedef float2 type; };
+
+// compaction of the bits of v selected by mask (order preserved)
+__device__ __forceinline__ int pext(int v, int mask) {
+  int r = 0, j = 0;
+#pragma unroll
+  for (int b = 0; b < 6; ++b)
+    if ((mask >> b) & 1) { r |= ((v >> b) & 1) << j; ++j; }
+  return r;
+}
+template <int MASK> __device__ __forceinline__ int pextc(int v) {
+  int r = 0, j = 0;
+#pragma unroll
+  for (int b = 0; b < 6; ++b)
+    if ((MASK >> b) & 1) { r |= ((v >> b) & 1) << j; ++j; }
+  return r;
+}
+
+// view of one event's shared memory
+template <class T, int NSLOT> struct View {
+  typedef typename V2<T>::type W;
+  const T* mom;    // [NMOM][4]
+  const T* ip;     // [NMOM]
+  W* ent;          // [4][NSLOT]
+  __device__ __forceinline__ cx<T> ld(int k, int i) const { const W w = ent[k * NSLOT + i]; return cx<T>(w.x, w.y); }
+  __device__ __forceinline__ void st(int k, int i, cx<T> c) const { W w; w.x = c.re; w.y = c.im; ent[k * NSLOT + i] = w; }
+  __device__ __forceinline__ Vec4<T> ldv(int i) const { Vec4<T> v; v.v[0] = ld(0, i); v.v[1] = ld(1, i); v.v[2] = ld(2, i); v.v[3] = ld(3, i); return v; }
+  __device__ __forceinline__ Spinor<T> lds(int i) const { Spinor<T> s; s.l[0] = ld(0, i); s.l[1] = ld(1, i); s.r[0] = ld(2, i); s.r[1] = ld(3, i); return s; }
+  __device__ __forceinline__ void stv(int i, const Vec4<T>& v) const { st(0, i, v.v[0]); st(1, i, v.v[1]); st(2, i, v.v[2]); st(3, i, v.v[3]); }
+  __device__ __forceinline__ void sts(int i, const Spinor<T>& s) const { st(0, i, s.l[0]); st(1, i, s.l[1]); st(2, i, s.r[0]); st(3, i, s.r[1]); }
+  __device__ __forceinline__ Mom<T> ldm(int m) const { Mom<T> p; p.v[0] = mom[4 * m]; p.v[1] = mom[4 * m + 1]; p.v[2] = mom[4 * m + 2]; p.v[3] = mom[4 * m + 3]; return p; }
+};
+
+// ---------------------------------------------------------------------------------------------------
+// one task = one (node, helicity variant v) of one event
+// ---------------------------------------------------------------------------------------------------
+template <class P, class T, int KIND> struct Task;
+
+template <class P, class T> struct Task<P, T, K_POLVEC> {
+  static __device__ __forceinline__ void run(const NodeDesc& d, int v, const View<T, P::NSLOT>& ev, T) {
+    ev.stv(d.out + v, polvec<T>(ev.ldm(d.mom), v ? 1 : -1, d.aux != 0));
+  }
+};
+template <class P, class T> struct Task<P, T, K_UBAR> {
+  static __device__ __forceinline__ void run(const NodeDesc& d, int v, const View<T, P::NSLOT>& ev, T mt) {
+    ev.sts(d.out + v, bar(spinor_u<T>(ev.ldm(d.mom), mt, v ? 1 : -1)));
+  }
+};
+template <class P, class T> struct Task<P, T, K_VSP> {
+  static __device__ __forceinline__ void run(const NodeDesc& d, int v, const View<T, P::NSLOT>& ev, T mt) {
+    ev.sts(d.out + v, spinor_v<T>(ev.ldm(d.mom), mt, v ? 1 : -1));
+  }
+};
+template <class P, class T> struct Task<P, T, K_VCUR> {
+  static __device__ __forceinline__ void run(const NodeDesc& d, int v, const View<T, P::NSLOT>& ev, T) {
+    Vec4<T> acc;
+#pragma unroll
+    for (int i = 0; i < 4; ++i) acc.v[i] = cx<T>((T)0, (T)0);
+    for (int it = 0; it < d.nterm; ++it) {
+      const TermDesc& t = P::term(d.aux + it);
+      const Vec4<T> A = ev.ldv(t.op[0].slot + pext(v, t.op[0].mask));
+      const Vec4<T> B = ev.ldv(t.op[1].slot + pext(v, t.op[1].mask));
+      if (t.type == 0) {
+        vvv_cur<T, false>(acc, (T)t.sign, A, ev.ldm(t.momA), B, ev.ldm(t.momB));
+      } else {
+        const Vec4<T> C = ev.ldv(t.op[2].slot + pext(v, t.op[2].mask));
+        vvvv_cur<T, false>(acc, (T)t.sign, t.type, A, B, C);
+      }
+    }
+    if (d.prop >= 0) acc = scale(ev.ip[d.prop], acc);
+    ev.stv(d.out + v, acc);
+  }
+};
+template <class P, class T> struct Task<P, T, K_ROWPROP> {   // psibar' = psibar Vslash (qslash+m) / (q^2-m^2)
+  static __device__ __forceinline__ void run(const NodeDesc& d, int v, const View<T, P::NSLOT>& ev, T mt) {
+    const Spinor<T> s = ev.lds(d.op[0].slot + pext(v, d.op[0].mask));
+    const Vec4<T> V = ev.ldv(d.op[1].slot + pext(v, d.op[1].mask));
+    ev.sts(d.out + v, ffv_row_prop(s, V, ev.ldm(d.mom), mt, ev.ip[d.prop]));
+  }
+};
+template <class P, class T> struct Task<P, T, K_COLPROP> {   // psi' = (qslash+m) Vslash psi / (q^2-m^2)
+  static __device__ __forceinline__ void run(const NodeDesc& d, int v, const View<T, P::NSLOT>& ev, T mt) {
+    const Spinor<T> s = ev.lds(d.op[0].slot + pext(v, d.op[0].mask));
+    const Vec4<T> V = ev.ldv(d.op[1].slot + pext(v, d.op[1].mask));
+    ev.sts(d.out + v, ffv_col_prop(s, V, ev.ldm(d.mom), mt, ev.ip[d.prop]));
+  }
+};
+template <class P, class T> struct Task<P, T, K_FFCUR> {     // G = (psibar gamma^mu psi) / K^2
+  static __device__ __forceinline__ void run(const NodeDesc& d, int v, const View<T, P::NSLOT>& ev, T) {
+    const Spinor<T> a = ev.lds(d.op[0].slot + pext(v, d.op[0].mask));
+    const Spinor<T> b = ev.lds(d.op[1].slot + pext(v, d.op[1].mask));
+    ev.stv(d.out + v, scale(ev.ip[d.prop], ff_current(a, b)));
+  }
+};
+template <class P, class T> struct Task<P, T, K_SLASHCOL> {  // half product Vslash psi (op0 = psi, op1 = V)
+  static __device__ __forceinline__ void run(const NodeDesc& d, int v, const View<T, P::NSLOT>& ev, T) {
+    const Spinor<T> s = ev.lds(d.op[0].slot + pext(v, d.op[0].mask));
+    const Vec4<T> V = ev.ldv(d.op[1].slot + pext(v, d.op[1].mask));
+    ev.sts(d.out + v, slash_col(slash_parts(V), s));
+  }
+};
+template <class P, class T> struct Task<P, T, K_SLASHROW> {  // half product psibar Vslash (op0 = psibar, op1 = V)
+  static __device__ __forceinline__ void run(const NodeDesc& d, int v, const View<T, P::NSLOT>& ev, T) {
+    const Spinor<T> s = ev.lds(d.op[0].slot + pext(v, d.op[0].mask));
+    const Vec4<T> V = ev.ldv(d.op[1].slot + pext(v, d.op[1].mask));
+    ev.sts(d.out + v, slash_row(slash_parts(V), s));
+  }
+};
+
+// shared memory of one CTA
+template <class P, class T> struct Smem {
+  typedef typename V2<T>::type W;
+  T* ext;   // [E][NPAR*4]   external momenta as loaded
+  T* mom;   // [E][NMOM][4]
+  T* ip;    // [E][NMOM]
+  W* ent;   // [E][4][NSLOT]
+  T* red;   // [NT/32]
+  __device__ __forceinline__ View<T, P::NSLOT> view(int e) const {
+    View<T, P::NSLOT> v;
+    v.mom = mom + e * P::NMOM * 4; v.ip = ip + e * P::NMOM; v.ent = ent + e * 4 * P::NSLOT;
+    return v;
+  }
+  static constexpr size_t bytes() {
+    return ((size_t)P::E * (P::NPAR * 4 + P::NMOM * 5) * sizeof(T) + 15) / 16 * 16 + (size_t)P::E * 4 * P::NSLOT * sizeof(W) + (P::NT / 32) * sizeof(T) + 16;
+  }
+};
+
+// task t of a group of `nfam` nodes that all have NB helicity bits: t -> (node, event, variant), variant fastest
+template <class P, class T, int KIND, int NB> __device__ __forceinline__ void run_group(const Smem<P, T>& s, int first_node, int nfam, int t, T mt) {
+  constexpr int PER = P::E << NB;
+  const int fam = t / PER;
+  if (fam >= nfam) return;
+  const int r = t - fam * PER;
+  Task<P, T, KIND>::run(P::node(first_node + fam), r & ((1 << NB) - 1), s.view(r >> NB), mt);
+}
+
+// ---------------------------------------------------------------------------------------------------
+// the kernel: grid = ceil(n / E) CTAs of NT = E * NHEL threads
+// ---------------------------------------------------------------------------------------------------
+template <class P, class T, bool PER_HEL>
+__global__ void __launch_bounds__(P::NT, P::MINB) sigmakin_recycle_kernel(Consts k, const T* __restrict__ mom, int64_t n, int64_t ld,
+                                                                          T* __restrict__ me, const T* __restrict__ psw,
+                                                                          T* __restrict__ evw, T* __restrict__ hel_out, uint64_t mask) {
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  typedef typename V2<T>::type W;
+  Smem<P, T> s;
+  s.ext = reinterpret_cast<T*>(smem_raw);
+  s.mom = s.ext + P::E * P::NPAR * 4;
+  s.ip = s.mom + P::E * P::NMOM * 4;
+  s.ent = reinterpret_cast<W*>(smem_raw + ((size_t)P::E * (P::NPAR * 4 + P::NMOM * 5) * sizeof(T) + 15) / 16 * 16);
+  s.red = reinterpret_cast<T*>(s.ent + P::E * 4 * P::NSLOT);
+  const int tid = threadIdx.x;
+  const int64_t ev0 = (int64_t)blockIdx.x * P::E;
+
+  // A5: momenta of the CTA's events (tail events re-read the last event and are not stored)
+  for (int i = tid; i < P::E * P::NPAR * 4; i += P::NT) {
+    const int e = i / (P::NPAR * 4), r = i - e * (P::NPAR * 4);
+    int64_t ge = ev0 + e;
+    if (ge >= n) ge = n - 1;
+    s.ext[i] = __ldg(mom + (int64_t)r * ld + ge);
+  }
+  __syncthreads();
+  // line momenta (signed sums of external momenta) and inverse propagator denominators, in double also
+  // for T = float (once per event; k_i.k_j cancels like theta^2 for collinear pairs, R19)
+  for (int i = tid; i < P::E * P::NMOM; i += P::NT) {
+    const int e = i / P::NMOM, m = i - e * P::NMOM;
+    const MomDef d = P::momdef(m);
+    double q[4] = {0, 0, 0, 0};
+#pragma unroll
+    for (int j = 0; j < P::NPAR; ++j) {
+      const double c = (double)d.c[j];
+#pragma unroll
+      for (int mu = 0; mu < 4; ++mu) q[mu] += c * (double)s.ext[(e * P::NPAR + j) * 4 + mu];
+    }
+#pragma unroll
+    for (int mu = 0; mu < 4; ++mu) s.mom[(e * P::NMOM + m) * 4 + mu] = (T)q[mu];
+    double den = fma(q[0], q[0], fma(-q[1], q[1], fma(-q[2], q[2], -q[3] * q[3])));
+    if (d.propkind == 2) den -= k.mt * k.mt;
+    s.ip[e * P::NMOM + m] = d.propkind ? (T)(1.0 / den) : (T)0;
+  }
+  __syncthreads();
+
+  const int el = tid / P::NHEL, h = tid - el * P::NHEL;
+  T me_h = P::template run<T>(s, tid, el, h, (T)k.mt);     // generated: producer steps + inner products + colour sum
+
+  const int64_t ge = ev0 + el;
+  if (PER_HEL) {
+    if (ge < n) hel_out[(int64_t)h * ld + ge] = me_h;
+    return;
+  }
+  if (!((mask >> h) & 1)) me_h = (T)0;
+  // A11: sum over the helicity lanes of the event (fixed order: butterfly inside the warp, then warps in order)
+  constexpr int LANES = P::NHEL < 32 ? P::NHEL : 32;
+#pragma unroll
+  for (int o = LANES / 2; o > 0; o >>= 1) me_h += __shfl_xor_sync(0xffffffffu, me_h, o);
+  if (P::NHEL > 32) {
+    if ((tid & 31) == 0) s.red[tid >> 5] = me_h;
+    __syncthreads();
+    if (h == 0) {
+      me_h = (T)0;
+#pragma unroll
+      for (int w = 0; w < P::NHEL / 32; ++w) me_h += s.red[el * (P::NHEL / 32) + w];
+    }
+  }
+  if (h == 0 && ge < n) {
+    const T r = me_h * (T)k.me_norm;
+    me[ge] = r;
+    if (evw != nullptr) evw[ge] = psw[ge] * r;
+  }
+}
+
+template <class P>
+cudaError_t launch_sigmakin_recycle(const mg_process* p, const MeArgs& a, cudaStream_t s) {
+  const unsigned g = (unsigned)((a.n + P::E - 1) / P::E);
+  const bool f64 = p->par.precision == MG_FP64;
+  cudaError_t e = cudaSuccess;
+#define MG_RC_LAUNCH(T, PH, ...)                                                                                    \
+  do {                                                                                                              \
+    auto kern = sigmakin_recycle_kernel<P, T, PH>;                                                                  \
+    const size_t sm = Smem<P, T>::bytes();                                                                          \
+    e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);                           \
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, 100);      \
+    if (e == cudaSuccess) kern<<<g, P::NT, sm, s>>>(__VA_ARGS__);                                                   \
+  } while (0)
+  if (a.hel_out) {
+    if (f64) MG_RC_LAUNCH(double, true, p->k, (const double*)a.mom, a.n, a.ld, nullptr, nullptr, nullptr, (double*)a.hel_out, 0);
+    else MG_RC_LAUNCH(float, true, p->k, (const float*)a.mom, a.n, a.ld, nullptr, nullptr, nullptr, (float*)a.hel_out, 0);
+  } else {
+    if (f64) MG_RC_LAUNCH(double, false, p->k, (const double*)a.mom, a.n, a.ld, (double*)a.me, (const double*)a.psw, (double*)a.evw, nullptr, a.mask);
+    else MG_RC_LAUNCH(float, false, p->k, (const float*)a.mom, a.n, a.ld, (float*)a.me, (const float*)a.psw, (float*)a.evw, nullptr, a.mask);
+  }
+#undef MG_RC_LAUNCH
+  if (e != cudaSuccess) return e;
+  return cudaGetLastError();
+}
+
+}  // namespace rc
+}  // namespace mg

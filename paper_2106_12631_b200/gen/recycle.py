@@ -1,0 +1,475 @@
+"""Helicity-recycling back-end of the gg -> t t~ (+ g, + g g) generator (csrc/recycle.cuh).
+
+Input: the diagram list of qcdgen.Generator (wavefunctions shared between diagrams; colour-flow
+decomposition).  Output: a PROGRAM for the kernel `sigmakin_recycle_kernel`:
+
+  nodes     every wavefunction as a node with the set of external legs whose helicity it depends on (`dep`);
+            a node with b legs has 2^b helicity variants, each computed once per event (a task);
+            besides the wavefunctions of the diagram list there are HALF PRODUCTS  Vslash.psi / psibar.Vslash
+            (so that a diagram closes as  row spinor . column spinor) and the all-gluon currents (closed with
+            the t t~ current G);
+  steps     producer steps (groups of nodes of the same kind and the same number of helicity bits, separated by
+            __syncthreads()) interleaved with per-helicity chunks of closures (inner products added into the
+            colour-flow sums); chunks bound the number of half products alive at once;
+  slots     shared-memory entries assigned by liveness (a node's entries are reused after its last reader);
+  tally     the explicit flop count of everything the kernel executes per event.
+
+The same program object is interpreted in numpy by tests/rc_interp.py (CPU check of tables, slots and signs
+against the oracle) and written out as CUDA by `emit()`.
+"""
+import itertools
+import os
+from collections import OrderedDict
+
+from . import qcdgen
+from .qcdgen import (F_FF_CUR, F_FFV_PROP, F_MDOT_VV, F_POLVEC, F_ROW_COL, F_SCALE, F_SLASH, F_SLASH_PARTS,
+                     F_SPINOR, F_VVV_CUR, F_VVVV_CUR)
+
+CSRC = qcdgen.CSRC
+PROC_NAME = {2: "RcGgtt", 3: "RcGgttg", 4: "RcGgttgg"}
+FILE_NAME = {2: "gen_rc_ggtt.cuh", 3: "gen_rc_ggttg.cuh", 4: "gen_rc_ggttgg.cuh"}
+KINDS = ["POLVEC", "UBAR", "VSP", "VCUR", "ROWPROP", "COLPROP", "FFCUR", "SLASHCOL", "SLASHROW"]
+KIND_ID = {k: i for i, k in enumerate(KINDS)}
+T_PART, TB_PART = 2, 3
+F_SETUP_MOM = 6 * 4 * 2 + 8 + 2      # one line momentum (6 fma x 4) + Minkowski square + mass shift + reciprocal
+
+
+class RNode:
+    def __init__(self, name, kind, dep, ops=(), **params):
+        self.name, self.kind = name, kind
+        self.dep = tuple(sorted(dep))
+        self.ops = list(ops)            # operand nodes (VCUR: see terms)
+        self.params = params            # mom, prop, outgoing, terms
+        self.level = 0
+        self.born = None                # step that writes it
+        self.last = None                # last step that reads it
+        self.slot = None                # first shared-memory entry
+
+    @property
+    def nbits(self):
+        return len(self.dep)
+
+    @property
+    def nvar(self):
+        return 1 << len(self.dep)
+
+    def operands(self):
+        if self.kind == "VCUR":
+            out = []
+            for t in self.params["terms"]:
+                out.extend(t["ops"])
+            return out
+        return self.ops
+
+    def local_mask(self, op):
+        """which of this node's variant bits select the operand's variant"""
+        assert set(op.dep) <= set(self.dep), (self.name, op.name)
+        return sum(1 << j for j, p in enumerate(self.dep) if p in op.dep)
+
+    def flops(self):
+        k = self.kind
+        if k == "POLVEC":
+            return F_POLVEC
+        if k in ("UBAR", "VSP"):
+            return F_SPINOR
+        if k == "VCUR":
+            f = sum(F_VVV_CUR if t["type"] == 0 else F_VVVV_CUR for t in self.params["terms"])
+            return f + (F_SCALE if self.params.get("prop") is not None else 0)
+        if k in ("ROWPROP", "COLPROP"):
+            return F_FFV_PROP
+        if k == "FFCUR":
+            return F_FF_CUR + F_SCALE
+        return F_SLASH_PARTS + F_SLASH
+
+
+class Closure:
+    def __init__(self, kind, a, b, flows):
+        self.kind, self.a, self.b, self.flows = kind, a, b, flows   # kind: 'DOTS' row.col | 'DOTV' vector.vector
+
+
+class Program:
+    def __init__(self, ng, chunk_budget=300):
+        self.ng = ng
+        g = self.g = qcdgen.Generator(ng)
+        self.npar = ng + 2
+        self.nhel = 1 << self.npar
+        self.E = max(1, 128 // self.nhel)
+        self.NT = self.E * self.nhel
+        self.gp = g.gl_particle
+        self._build_momenta()
+        self._build_nodes()
+        self._build_closures()
+        self._schedule(chunk_budget)
+        self._allocate()
+        self._tally()
+
+    # ------------------------------------------------------------------ momentum table
+    def _build_momenta(self):
+        g, ng, npar = self.g, self.ng, self.npar
+        self.mom_names, self.mom_defs = [], []          # defs: (coefficients[npar], propkind)
+
+        def add(name, coef, kind):
+            self.mom_names.append(name)
+            self.mom_defs.append((tuple(coef), kind))
+
+        for i in range(npar):
+            add("p%d" % i, [1 if j == i else 0 for j in range(npar)], 0)
+
+        def kcoef(S):
+            c = [0] * npar
+            for gi in S:
+                c[self.gp[gi]] = 1 if gi < 2 else -1     # all gluon momenta incoming
+            return c
+
+        self.kidx = {}
+        for size in range(1, ng):
+            for S in map(frozenset, itertools.combinations(range(ng), size)):
+                self.kidx[S] = len(self.mom_names)
+                add("K" + "".join(map(str, sorted(S))), kcoef(S), 1 if size > 1 else 0)
+        self.qidx = {}
+        for name, (side, prev, st, absorbed) in g.quark_wfs.items():
+            key = (side, absorbed)
+            if key in self.qidx:
+                continue
+            c = kcoef(absorbed)
+            if side == "L":
+                c = [-x for x in c]
+                c[T_PART] += 1                           # q = p_t - K
+            else:
+                c[TB_PART] -= 1                          # q = K - p_tbar
+            self.qidx[key] = len(self.mom_names)
+            add("q%s%s" % (side, "".join(map(str, sorted(absorbed)))), c, 2)
+        c = [0] * npar
+        c[T_PART] = c[TB_PART] = 1
+        self.kf = len(self.mom_names)
+        add("Kf", c, 1)
+
+    # ------------------------------------------------------------------ nodes of the diagram list
+    def _build_nodes(self):
+        g = self.g
+        self.nodes = OrderedDict()
+
+        def add(n):
+            assert n.name not in self.nodes
+            self.nodes[n.name] = n
+            return n
+
+        for gi in range(self.ng):
+            add(RNode("eps%d" % gi, "POLVEC", [self.gp[gi]], mom=self.gp[gi], outgoing=gi >= 2))
+        add(RNode("ubar", "UBAR", [T_PART], mom=T_PART))
+        add(RNode("v", "VSP", [TB_PART], mom=TB_PART))
+        for st in g.struct_order:
+            add(self._vcur(st.name, st, st.terms, prop=self.kidx[st.subset]))
+        for name, (side, prev, st, absorbed) in g.quark_wfs.items():
+            a, b = self.nodes[prev], self.nodes[st.name]
+            q = self.qidx[(side, absorbed)]
+            add(RNode(name, "ROWPROP" if side == "L" else "COLPROP", set(a.dep) | set(b.dep), [a, b], mom=q, prop=q))
+        add(RNode("G", "FFCUR", [T_PART, TB_PART], [self.nodes["ubar"], self.nodes["v"]], prop=self.kf))
+
+    def _vcur(self, name, st_or_subset, terms, prop):
+        subset = st_or_subset.subset if hasattr(st_or_subset, "subset") else st_or_subset
+        out = []
+        for t in terms:
+            if t[1] in ("V3", "V3G"):
+                a, b = t[2], t[3]
+                out.append(dict(type=0, sign=t[0], ops=[self.nodes[a.name], self.nodes[b.name]],
+                                momA=self.kidx[a.subset], momB=self.kidx[b.subset]))
+            else:
+                which, a, b, c = t[2], t[3], t[4], t[5]
+                out.append(dict(type=which, sign=t[0], ops=[self.nodes[a.name], self.nodes[b.name], self.nodes[c.name]],
+                                momA=0, momB=0))
+        return RNode(name, "VCUR", [self.gp[gi] for gi in subset], terms=out, prop=prop)
+
+    # ------------------------------------------------------------------ closures as inner products
+    def _build_closures(self):
+        g = self.g
+        self.closures = []
+        self.half = OrderedDict()       # half-product and all-gluon nodes
+        nfull = 0
+        for col, terms in g.closures:
+            flows = [(g.flow_index[w], c) for w, c in sorted(col.items())]
+            if terms[0][1] == "FFV":
+                assert len(terms) == 1 and terms[0][0] == 1
+                L, V, R = self.nodes[terms[0][2]], self.nodes[terms[0][3].name], self.nodes[terms[0][4]]
+                cdep, rdep = set(V.dep) | set(R.dep), set(L.dep) | set(V.dep)
+                if len(cdep) <= len(rdep):
+                    key = "W_%s_%s" % (V.name, R.name)
+                    if key not in self.half:
+                        self.half[key] = RNode(key, "SLASHCOL", cdep, [R, V])
+                    self.closures.append(Closure("DOTS", L, self.half[key], flows))
+                else:
+                    key = "U_%s_%s" % (L.name, V.name)
+                    if key not in self.half:
+                        self.half[key] = RNode(key, "SLASHROW", rdep, [L, V])
+                    self.closures.append(Closure("DOTS", self.half[key], R, flows))
+            else:
+                key = "JF%d" % nfull
+                nfull += 1
+                self.half[key] = self._vcur(key, frozenset(range(self.ng)), terms, prop=None)
+                self.closures.append(Closure("DOTV", self.half[key], self.nodes["G"], flows))
+
+    # ------------------------------------------------------------------ steps
+    def _schedule(self, budget):
+        # levels of the base nodes
+        for n in self.nodes.values():
+            n.level = 1 + max([o.level for o in n.operands()], default=-1)
+        nlev = 1 + max(n.level for n in self.nodes.values())
+        self.steps = []                                   # ('P', [nodes]) | ('F', [closures])
+        for lv in range(nlev):
+            self.steps.append(("P", [n for n in self.nodes.values() if n.level == lv]))
+        # chunks of closures: classes by (kind of new node, its number of helicity bits), small classes merged
+        def new_node(c):
+            return c.a if c.a.name in self.half else (c.b if c.b.name in self.half else None)
+
+        classes = OrderedDict()
+        for c in self.closures:
+            nn = new_node(c)
+            classes.setdefault((nn.nbits, nn.kind), []).append(c)
+        chunks, cur, cur_n = [], [], 0
+        for key in sorted(classes):
+            cl = classes[key]
+            nnew = sum(n.nvar for n in {new_node(c).name: new_node(c) for c in cl}.values())
+            if cur and cur_n + nnew > budget:
+                chunks.append(cur)
+                cur, cur_n = [], 0
+            cur = cur + cl
+            cur_n += nnew
+        if cur:
+            chunks.append(cur)
+        for ch in chunks:
+            hp = OrderedDict()
+            for c in ch:
+                nn = new_node(c)
+                hp[nn.name] = nn
+            self.steps.append(("P", list(hp.values())))
+            # closures sharing the second operand are adjacent: it is loaded once
+            self.steps.append(("F", sorted(ch, key=lambda c: (c.b.name, c.a.name))))
+        # birth / last use
+        for si, (kind, items) in enumerate(self.steps):
+            if kind == "P":
+                for n in items:
+                    n.born = si
+                    for o in n.operands():
+                        o.last = si
+            else:
+                for c in items:
+                    c.a.last = si
+                    c.b.last = si
+        self.all_nodes = [n for kind, items in self.steps if kind == "P" for n in items]
+        for n in self.all_nodes:
+            assert n.last is not None and n.last > n.born, n.name
+            for o in n.operands():
+                assert o.born < n.born
+
+    # ------------------------------------------------------------------ shared-memory entries by liveness
+    def _allocate(self):
+        live = []          # (slot, size, last)
+        self.nslot = 0
+        for n in self.all_nodes:
+            live = [iv for iv in live if iv[2] >= n.born]          # entries whose last reader ran in an earlier step are free
+            align = min(n.nvar, 8)
+            pos = 0
+            for s, size, _ in sorted(live):
+                if pos + n.nvar <= s:
+                    break
+                pos = max(pos, (s + size + align - 1) // align * align)
+            n.slot = pos
+            live.append((pos, n.nvar, n.last))
+            self.nslot = max(self.nslot, pos + n.nvar)
+        self.nslot = (self.nslot + 7) // 8 * 8
+
+    # ------------------------------------------------------------------ flops per event (everything executed)
+    def _tally(self):
+        self.flops_nodes = sum(n.nvar * n.flops() for n in self.all_nodes)
+        self.flops_setup = len(self.mom_defs) * F_SETUP_MOM
+        num, den = self.g.colour_matrix()
+        self.num, self.den = num, den
+        nf = len(self.g.flows)
+        f = 0
+        seen = set()
+        for c in self.closures:
+            f += F_ROW_COL if c.kind == "DOTS" else F_MDOT_VV
+            for fl, sg in c.flows:
+                if fl in seen:
+                    f += 2
+                seen.add(fl)
+        for a in range(nf):
+            f += 2 + 4 + 4 * sum(1 for b in range(a + 1, nf) if num[a][b] != 0)
+        f += 1
+        self.flops_hel = f
+        self.flops_event = self.flops_setup + self.flops_nodes + self.nhel * self.flops_hel + self.nhel + 1
+
+    # ------------------------------------------------------------------ groups of a producer step
+    @staticmethod
+    def groups(nodes):
+        gr = OrderedDict()
+        for n in nodes:
+            gr.setdefault((n.kind, n.nbits), []).append(n)
+        return gr
+
+
+# ----------------------------------------------------------------------------------------------
+# CUDA emission
+# ----------------------------------------------------------------------------------------------
+def emit(prog):
+    g = prog.g
+    ng, npar, nf = prog.ng, prog.npar, len(g.flows)
+    name = PROC_NAME[ng]
+    tag = name[2:].lower()
+    L = []
+    w = L.append
+    w("// GENERATED by paper_2106_12631_b200/gen/recycle.py — do not edit.")
+    w("// g g -> t t~%s with helicity recycling (csrc/recycle.cuh; DESIGN.md §5.4): %d diagrams, %d colour flows;" % (" g" * (ng - 2), g.n_diag, nf))
+    w("// %d nodes / %d tasks per event (%d half products or all-gluon currents), %d inner products per helicity," %
+      (len(prog.all_nodes), sum(n.nvar for n in prog.all_nodes), len(prog.half), len(prog.closures)))
+    w("// %d shared-memory entries per event, %d steps.  Flops per event: %d (setup %d, tasks %d, per helicity %d x %d)." %
+      (prog.nslot, len(prog.steps), prog.flops_event, prog.flops_setup, prog.flops_nodes, prog.nhel, prog.flops_hel))
+    w("#pragma once")
+    w('#include "recycle.cuh"')
+    w("namespace mg {")
+    # tables: nodes in step/group order
+    order, index = [], {}
+    for kind, items in prog.steps:
+        if kind != "P":
+            continue
+        for (k, nb), ns in Program.groups(items).items():
+            for n in ns:
+                index[n.name] = len(order)
+                order.append(n)
+    terms = []
+    w("__constant__ rc::MomDef kRcMom_%s[%d] = {" % (tag, len(prog.mom_defs)))
+    for nm, (coef, kind) in zip(prog.mom_names, prog.mom_defs):
+        c6 = list(coef) + [0] * (6 - len(coef))
+        w("  {{%s}, %d, 0},   // %s" % (", ".join(str(x) for x in c6), kind, nm))
+    w("};")
+    node_lines = []
+    for n in order:
+        ops = [(0, 0), (0, 0)]
+        aux, nterm = 0, 0
+        if n.kind == "VCUR":
+            aux, nterm = len(terms), len(n.params["terms"])
+            for t in n.params["terms"]:
+                o = [(x.slot, n.local_mask(x)) for x in t["ops"]] + [(0, 0)] * (3 - len(t["ops"]))
+                terms.append("  {%d, %d, %d, %d, {%s}},   // %s: %s" % (t["type"], t["sign"], t["momA"], t["momB"],
+                             ", ".join("{%d, %d}" % x for x in o), n.name, " ".join(x.name for x in t["ops"])))
+        else:
+            for i, x in enumerate(n.ops):
+                ops[i] = (x.slot, n.local_mask(x))
+            if n.kind == "POLVEC":
+                aux = 1 if n.params["outgoing"] else 0
+        prop = n.params.get("prop")
+        node_lines.append("  {%d, %d, %d, %d, %d, {%s}},   // %d %s %s dep %s" % (
+            n.slot, -1 if prop is None else prop, n.params.get("mom", 0), aux, nterm,
+            ", ".join("{%d, %d}" % x for x in ops), index[n.name], n.kind, n.name, "".join(map(str, n.dep))))
+    w("__constant__ rc::TermDesc kRcTerm_%s[%d] = {" % (tag, max(1, len(terms))))
+    for t in terms or ["  {0, 0, 0, 0, {{0, 0}, {0, 0}, {0, 0}}},"]:
+        w(t)
+    w("};")
+    w("__constant__ rc::NodeDesc kRcNode_%s[%d] = {" % (tag, len(order)))
+    for l in node_lines:
+        w(l)
+    w("};")
+    w("struct %s {" % name)
+    w("  static constexpr int NPAR = %d, NHEL = %d, NFLOW = %d, E = %d, NT = %d, MINB = %d;" % (npar, prog.nhel, nf, prog.E, prog.NT, 3))
+    w("  static constexpr int NMOM = %d, NSLOT = %d;" % (len(prog.mom_defs), prog.nslot))
+    w("  static __device__ __forceinline__ const rc::NodeDesc& node(int i) { return kRcNode_%s[i]; }" % tag)
+    w("  static __device__ __forceinline__ const rc::TermDesc& term(int i) { return kRcTerm_%s[i]; }" % tag)
+    w("  static __device__ __forceinline__ rc::MomDef momdef(int i) { return kRcMom_%s[i]; }" % tag)
+    w("")
+    w("  // producer steps, inner products, colour sum: |M|^2 of helicity h of event el (no g_s^(2 n_g)/denominator)")
+    w("  template <class T> static __device__ __forceinline__ T run(const rc::Smem<%s, T>& s, int tid, int el, int h, T mt) {" % name)
+    w("    const rc::View<T, NSLOT> ev = s.view(el);")
+    w("    cx<T> jamp[NFLOW];")
+    seen = set()
+    for si, (kind, items) in enumerate(prog.steps):
+        if kind == "P":
+            gr = Program.groups(items)
+            bounds, b = [], 0
+            for (k, nb), ns in gr.items():
+                cnt = len(ns) * (prog.E << nb)
+                pad = (cnt + 31) // 32 * 32
+                bounds.append((k, nb, index[ns[0].name], len(ns), b, b + pad))
+                b += pad
+            w("    // step %d: %s" % (si, ", ".join("%d x %s/%d bits" % (len(ns), k, nb) for (k, nb), ns in gr.items())))
+            w("    for (int t = tid; t < %d; t += NT) {" % b)
+            for i, (k, nb, first, nfam, lo, hi) in enumerate(bounds):
+                cond = "" if len(bounds) == 1 else ("if (t < %d) " % hi if i == 0 else ("else if (t < %d) " % hi if i < len(bounds) - 1 else "else "))
+                w("      %src::run_group<%s, T, rc::K_%s, %d>(s, %d, %d, t - %d, mt);" % (cond, name, k, nb, first, nfam, lo))
+            w("    }")
+            w("    __syncthreads();")
+        else:
+            w("    // step %d: %d inner products" % (si, len(items)))
+            cur_b = None
+            w("    {")
+            for c in items:
+                ld_b = "ldv" if c.kind == "DOTV" else "lds"
+                typ = "Vec4<T>" if c.kind == "DOTV" else "Spinor<T>"
+                if c.b.name != cur_b:
+                    if cur_b is not None:
+                        w("      }")
+                    w("      { const %s B = ev.%s(%d + rc::pextc<%d>(h));   // %s" % (typ, ld_b, c.b.slot, _hmask(c.b), c.b.name))
+                    cur_b = c.b.name
+                fn = "mdot" if c.kind == "DOTV" else "row_col"
+                w("        { const cx<T> a = %s(ev.%s(%d + rc::pextc<%d>(h)), B);   // %s" % (fn, ld_b, c.a.slot, _hmask(c.a), c.a.name))
+                for fl, sg in c.flows:
+                    if fl not in seen:
+                        seen.add(fl)
+                        w("          jamp[%d] = %sa;" % (fl, "" if sg > 0 else "-"))
+                    else:
+                        w("          jamp[%d] = jamp[%d] %s a;" % (fl, fl, "+" if sg > 0 else "-"))
+                w("        }")
+            w("      }")
+            w("    }")
+            if si != len(prog.steps) - 1:
+                w("    __syncthreads();")
+    assert len(seen) == nf
+    num, den = prog.num, prog.den
+    w("    // A10: colour sum  sum_f C_ff |J_f|^2 + 2 sum_{f<g} C_fg Re(J_f^* J_g),  C = numerators / %d" % den)
+    w("    T me = (T)0;")
+    for f in range(nf):
+        w("    { T zr = (T)%d * jamp[%d].re, zi = (T)%d * jamp[%d].im;" % (num[f][f], f, num[f][f], f))
+        for hh in range(f + 1, nf):
+            if num[f][hh] == 0:
+                continue
+            w("      zr = fma_<T>((T)%d, jamp[%d].re, zr); zi = fma_<T>((T)%d, jamp[%d].im, zi);" % (2 * num[f][hh], hh, 2 * num[f][hh], hh))
+        w("      me = fma_<T>(jamp[%d].re, zr, fma_<T>(jamp[%d].im, zi, me)); }" % (f, f))
+    w("    return me * (T)%s;" % repr(1.0 / den))
+    w("  }")
+    w("};")
+    w("}  // namespace mg")
+    return "\n".join(L) + "\n"
+
+
+def _hmask(n):
+    return sum(1 << p for p in n.dep)
+
+
+def generate(ng):
+    prog = Program(ng)
+    return prog, emit(prog)
+
+
+def tables(progs):
+    out = "// GENERATED by paper_2106_12631_b200/gen/recycle.py — do not edit.\n#pragma once\nnamespace mg {\n"
+    for ng, prog in progs:
+        out += "static const long kFlopsRecycle_%d = %d;   // per event: setup %d + tasks %d + %d helicities x %d + reduction\n" % (
+            ng, prog.flops_event, prog.flops_setup, prog.flops_nodes, prog.nhel, prog.flops_hel)
+    return out + "}  // namespace mg\n"
+
+
+def main():
+    progs = []
+    for ng in (2, 3, 4):
+        prog, src = generate(ng)
+        progs.append((ng, prog))
+        with open(os.path.join(CSRC, FILE_NAME[ng]), "w") as f:
+            f.write(src)
+        print("ng=%d: %d nodes, %d tasks/event, %d closures, %d slots (%.1f KB/event FP64), %d steps, flops/event %d (per hel %d)" %
+              (ng, len(prog.all_nodes), sum(n.nvar for n in prog.all_nodes), len(prog.closures), prog.nslot,
+               prog.nslot * 64 / 1024.0, len(prog.steps), prog.flops_event, prog.flops_hel))
+    with open(os.path.join(CSRC, "gen_rc_tables.cuh"), "w") as f:
+        f.write(tables(progs))
+
+
+if __name__ == "__main__":
+    main()
