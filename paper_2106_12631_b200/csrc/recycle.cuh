@@ -27,20 +27,23 @@
 namespace mg {
 namespace rc {
 
-enum Kind { K_POLVEC = 0, K_UBAR = 1, K_VSP = 2, K_VCUR = 3, K_ROWPROP = 4, K_COLPROP = 5, K_FFCUR = 6, K_SLASHCOL = 7, K_SLASHROW = 8 };
+enum Kind { K_POLVEC = 0, K_UBAR = 1, K_VSP = 2, K_VCUR = 3, K_ROWPROP = 4, K_COLPROP = 5, K_FFCUR = 6, K_SLASHCOL = 7, K_SLASHROW = 8, K_EXT = 9 };
 
-struct Op { short slot; short mask; };   // operand: first entry, and which of the consumer's variant bits select its variant
+// operand word: low 16 bits = first entry of the operand node, high 16 bits = 4 * mask, where mask says which of
+// the consumer's variant bits select the operand's variant (pext through the per-variant table, see pext4)
+typedef unsigned int Op;
 struct NodeDesc {
   short out;        // first entry of the result
   short prop;       // index into the inverse-propagator table, -1: none
-  short mom;        // momentum-table index (line momentum of a propagator; particle momentum of an external)
-  short aux;        // K_POLVEC: 1 = outgoing;  K_VCUR: first term
-  short nterm;      // K_VCUR: number of terms
+  short mom;        // momentum-table index (line momentum of a propagator; particle index of an external)
+  short aux;        // K_EXT: 0/1 = incoming/outgoing polarisation vector, 2 = ubar, 3 = v;  K_VCUR: first term
+  int nterm;        // K_VCUR: number of terms
   Op op[2];
 };
 struct TermDesc {   // one term of a gluon current: type 0: V3(A,kA,B,kB);  1..3: four-gluon structure `type`(A,B,C)
-  short type, sign;
-  short momA, momB;
+  short type;
+  short momA, momB, pad;
+  unsigned int signbit;   // 0 or 0x80000000: the term enters with sign -1
   Op op[3];
 };
 struct MomDef { signed char c[6]; signed char propkind; signed char pad; };   // momentum = sum_i c[i] p_i ; 0 none, 1: 1/q^2, 2: 1/(q^2-mt^2)
@@ -57,6 +60,12 @@ __device__ __forceinline__ int pext(int v, int mask) {
     if ((mask >> b) & 1) { r |= ((v >> b) & 1) << j; ++j; }
   return r;
 }
+// pext of a variant index v < 16 with any mask < 16 from ONE 64-bit word per v: nibble `mask` of kPext4[v] is
+// pext(v, mask).  A thread's v is fixed within a group (v = low bits of the thread index), so the word is
+// fetched once per task and every operand costs a shift and an AND.
+__device__ __forceinline__ int entry_of(Op op, unsigned long long pt) {
+  return (int)(op & 0xffffu) + (int)((pt >> (op >> 16)) & 15ull);
+}
 template <int MASK> __device__ __forceinline__ int pextc(int v) {
   int r = 0, j = 0;
 #pragma unroll
@@ -68,8 +77,9 @@ template <int MASK> __device__ __forceinline__ int pextc(int v) {
 // view of one event's shared memory
 template <class T, int NSLOT> struct View {
   typedef typename V2<T>::type W;
-  const T* mom;    // [NMOM][4]
-  const T* ip;     // [NMOM]
+  const T* ext;    // [NPAR][4]  external momenta as loaded
+  const T* mom;    // [NMOM][4]  line momenta
+  const T* ip;     // [NMOM]     inverse propagator denominators
   W* ent;          // [4][NSLOT]
   __device__ __forceinline__ cx<T> ld(int k, int i) const { const W w = ent[k * NSLOT + i]; return cx<T>(w.x, w.y); }
   __device__ __forceinline__ void st(int k, int i, cx<T> c) const { W w; w.x = c.re; w.y = c.im; ent[k * NSLOT + i] = w; }
@@ -77,100 +87,124 @@ template <class T, int NSLOT> struct View {
   __device__ __forceinline__ Spinor<T> lds(int i) const { Spinor<T> s; s.l[0] = ld(0, i); s.l[1] = ld(1, i); s.r[0] = ld(2, i); s.r[1] = ld(3, i); return s; }
   __device__ __forceinline__ void stv(int i, const Vec4<T>& v) const { st(0, i, v.v[0]); st(1, i, v.v[1]); st(2, i, v.v[2]); st(3, i, v.v[3]); }
   __device__ __forceinline__ void sts(int i, const Spinor<T>& s) const { st(0, i, s.l[0]); st(1, i, s.l[1]); st(2, i, s.r[0]); st(3, i, s.r[1]); }
-  __device__ __forceinline__ Mom<T> ldm(int m) const { Mom<T> p; p.v[0] = mom[4 * m]; p.v[1] = mom[4 * m + 1]; p.v[2] = mom[4 * m + 2]; p.v[3] = mom[4 * m + 3]; return p; }
+  __device__ __forceinline__ Mom<T> ldm(int m) const { return ld4(mom + 4 * m); }
+  __device__ __forceinline__ Mom<T> ldx(int i) const { return ld4(ext + 4 * i); }
+  static __device__ __forceinline__ Mom<T> ld4(const T* q) {
+    const W a = reinterpret_cast<const W*>(q)[0], b = reinterpret_cast<const W*>(q)[1];
+    Mom<T> p; p.v[0] = a.x; p.v[1] = a.y; p.v[2] = b.x; p.v[3] = b.y; return p;
+  }
 };
 
 // ---------------------------------------------------------------------------------------------------
-// one task = one (node, helicity variant v) of one event
+// one task = one (node, helicity variant v) of one event.  pt = kPext4 word of v (see entry_of).
 // ---------------------------------------------------------------------------------------------------
-template <class P, class T, int KIND> struct Task;
+__device__ __forceinline__ double flip(double x, unsigned int signbit) {
+  return __hiloint2double(__double2hiint(x) ^ (int)signbit, __double2loint(x));
+}
+__device__ __forceinline__ float flip(float x, unsigned int signbit) { return __int_as_float(__float_as_int(x) ^ (int)signbit); }
+template <class T> __device__ __forceinline__ cx<T> flip(cx<T> a, unsigned int signbit) { return cx<T>(flip(a.re, signbit), flip(a.im, signbit)); }
 
-template <class P, class T> struct Task<P, T, K_POLVEC> {
-  static __device__ __forceinline__ void run(const NodeDesc& d, int v, const View<T, P::NSLOT>& ev, T) {
-    ev.stv(d.out + v, polvec<T>(ev.ldm(d.mom), v ? 1 : -1, d.aux != 0));
-  }
-};
-template <class P, class T> struct Task<P, T, K_UBAR> {
-  static __device__ __forceinline__ void run(const NodeDesc& d, int v, const View<T, P::NSLOT>& ev, T mt) {
-    ev.sts(d.out + v, bar(spinor_u<T>(ev.ldm(d.mom), mt, v ? 1 : -1)));
-  }
-};
-template <class P, class T> struct Task<P, T, K_VSP> {
-  static __device__ __forceinline__ void run(const NodeDesc& d, int v, const View<T, P::NSLOT>& ev, T mt) {
-    ev.sts(d.out + v, spinor_v<T>(ev.ldm(d.mom), mt, v ? 1 : -1));
-  }
-};
-template <class P, class T> struct Task<P, T, K_VCUR> {
-  static __device__ __forceinline__ void run(const NodeDesc& d, int v, const View<T, P::NSLOT>& ev, T) {
-    Vec4<T> acc;
+// acc += (+-) V3(J1,k1,J2,k2): helas.cuh vvv_cur with the sign applied as a sign-bit flip of the three scalars
+template <class T> __device__ __forceinline__ void vvv_acc(Vec4<T>& acc, unsigned int signbit, const Vec4<T>& J1, Mom<T> k1, const Vec4<T>& J2, Mom<T> k2) {
+  Mom<T> d, e, f;
 #pragma unroll
-    for (int i = 0; i < 4; ++i) acc.v[i] = cx<T>((T)0, (T)0);
-    for (int it = 0; it < d.nterm; ++it) {
-      const TermDesc& t = P::term(d.aux + it);
-      const Vec4<T> A = ev.ldv(t.op[0].slot + pext(v, t.op[0].mask));
-      const Vec4<T> B = ev.ldv(t.op[1].slot + pext(v, t.op[1].mask));
-      if (t.type == 0) {
-        vvv_cur<T, false>(acc, (T)t.sign, A, ev.ldm(t.momA), B, ev.ldm(t.momB));
-      } else {
-        const Vec4<T> C = ev.ldv(t.op[2].slot + pext(v, t.op[2].mask));
-        vvvv_cur<T, false>(acc, (T)t.sign, t.type, A, B, C);
-      }
+  for (int i = 0; i < 4; ++i) { d.v[i] = k1.v[i] - k2.v[i]; e.v[i] = fma_<T>((T)2, k2.v[i], k1.v[i]); f.v[i] = -fma_<T>((T)2, k1.v[i], k2.v[i]); }
+  const cx<T> j12 = flip(mdot(J1, J2), signbit);
+  const cx<T> a = flip(mdot(J1, e), signbit);
+  const cx<T> b = flip(mdot(J2, f), signbit);
+#pragma unroll
+  for (int i = 0; i < 4; ++i) acc.v[i] = cfma(b, J1.v[i], cfma(a, J2.v[i], rfma(d.v[i], j12, acc.v[i])));
+}
+// acc += (+-) [ (A.B) C - (C.B) A ]: every four-gluon structure of helas.cuh vvvv_cur is this form after a
+// permutation of its operands, done by the generator (s1: (A,C,B), s2: (A,B,C), s3: (B,A,C))
+template <class T> __device__ __forceinline__ void vvvv_acc(Vec4<T>& acc, unsigned int signbit, const Vec4<T>& A, const Vec4<T>& B, const Vec4<T>& C) {
+  const cx<T> p = flip(mdot(A, B), signbit), q = flip(mdot(C, B), signbit);
+#pragma unroll
+  for (int i = 0; i < 4; ++i) acc.v[i] = cfms(q, A.v[i], cfma(p, C.v[i], acc.v[i]));
+}
+
+template <class P, class T, int KIND> struct Task;
+#define MG_RC_TASK(K) template <class P, class T> struct Task<P, T, K> { \
+  static __device__ __forceinline__ void run(const NodeDesc& d, int v, unsigned long long pt, const View<T, P::NSLOT>& ev, T mt)
+
+MG_RC_TASK(K_POLVEC) { ev.stv(d.out + v, polvec<T>(ev.ldx(d.mom), v ? 1 : -1, d.aux != 0)); } };
+MG_RC_TASK(K_UBAR) { ev.sts(d.out + v, bar(spinor_u<T>(ev.ldx(d.mom), mt, v ? 1 : -1))); } };
+MG_RC_TASK(K_VSP) { ev.sts(d.out + v, spinor_v<T>(ev.ldx(d.mom), mt, v ? 1 : -1)); } };
+MG_RC_TASK(K_EXT) {      // external wavefunctions of one warp: polarisation vectors and the two spinors
+  const Mom<T> p = ev.ldx(d.mom);
+  if (d.aux < 2) ev.stv(d.out + v, polvec<T>(p, v ? 1 : -1, d.aux != 0));
+  else if (d.aux == 2) ev.sts(d.out + v, bar(spinor_u<T>(p, mt, v ? 1 : -1)));
+  else ev.sts(d.out + v, spinor_v<T>(p, mt, v ? 1 : -1));
+} };
+MG_RC_TASK(K_VCUR) {
+  Vec4<T> acc;
+#pragma unroll
+  for (int i = 0; i < 4; ++i) acc.v[i] = cx<T>((T)0, (T)0);
+  for (int it = 0; it < d.nterm; ++it) {
+    const TermDesc& t = P::term(d.aux + it);
+    const Vec4<T> A = ev.ldv(entry_of(t.op[0], pt));
+    const Vec4<T> B = ev.ldv(entry_of(t.op[1], pt));
+    if (t.type == 0) {
+      vvv_acc<T>(acc, t.signbit, A, ev.ldm(t.momA), B, ev.ldm(t.momB));
+    } else {
+      const Vec4<T> C = ev.ldv(entry_of(t.op[2], pt));
+      vvvv_acc<T>(acc, t.signbit, A, B, C);
     }
-    if (d.prop >= 0) acc = scale(ev.ip[d.prop], acc);
-    ev.stv(d.out + v, acc);
   }
-};
-template <class P, class T> struct Task<P, T, K_ROWPROP> {   // psibar' = psibar Vslash (qslash+m) / (q^2-m^2)
-  static __device__ __forceinline__ void run(const NodeDesc& d, int v, const View<T, P::NSLOT>& ev, T mt) {
-    const Spinor<T> s = ev.lds(d.op[0].slot + pext(v, d.op[0].mask));
-    const Vec4<T> V = ev.ldv(d.op[1].slot + pext(v, d.op[1].mask));
-    ev.sts(d.out + v, ffv_row_prop(s, V, ev.ldm(d.mom), mt, ev.ip[d.prop]));
-  }
-};
-template <class P, class T> struct Task<P, T, K_COLPROP> {   // psi' = (qslash+m) Vslash psi / (q^2-m^2)
-  static __device__ __forceinline__ void run(const NodeDesc& d, int v, const View<T, P::NSLOT>& ev, T mt) {
-    const Spinor<T> s = ev.lds(d.op[0].slot + pext(v, d.op[0].mask));
-    const Vec4<T> V = ev.ldv(d.op[1].slot + pext(v, d.op[1].mask));
-    ev.sts(d.out + v, ffv_col_prop(s, V, ev.ldm(d.mom), mt, ev.ip[d.prop]));
-  }
-};
-template <class P, class T> struct Task<P, T, K_FFCUR> {     // G = (psibar gamma^mu psi) / K^2
-  static __device__ __forceinline__ void run(const NodeDesc& d, int v, const View<T, P::NSLOT>& ev, T) {
-    const Spinor<T> a = ev.lds(d.op[0].slot + pext(v, d.op[0].mask));
-    const Spinor<T> b = ev.lds(d.op[1].slot + pext(v, d.op[1].mask));
-    ev.stv(d.out + v, scale(ev.ip[d.prop], ff_current(a, b)));
-  }
-};
-template <class P, class T> struct Task<P, T, K_SLASHCOL> {  // half product Vslash psi (op0 = psi, op1 = V)
-  static __device__ __forceinline__ void run(const NodeDesc& d, int v, const View<T, P::NSLOT>& ev, T) {
-    const Spinor<T> s = ev.lds(d.op[0].slot + pext(v, d.op[0].mask));
-    const Vec4<T> V = ev.ldv(d.op[1].slot + pext(v, d.op[1].mask));
-    ev.sts(d.out + v, slash_col(slash_parts(V), s));
-  }
-};
-template <class P, class T> struct Task<P, T, K_SLASHROW> {  // half product psibar Vslash (op0 = psibar, op1 = V)
-  static __device__ __forceinline__ void run(const NodeDesc& d, int v, const View<T, P::NSLOT>& ev, T) {
-    const Spinor<T> s = ev.lds(d.op[0].slot + pext(v, d.op[0].mask));
-    const Vec4<T> V = ev.ldv(d.op[1].slot + pext(v, d.op[1].mask));
-    ev.sts(d.out + v, slash_row(slash_parts(V), s));
-  }
-};
+  if (d.prop >= 0) acc = scale(ev.ip[d.prop], acc);
+  ev.stv(d.out + v, acc);
+} };
+MG_RC_TASK(K_ROWPROP) {   // psibar' = psibar Vslash (qslash+m) / (q^2-m^2)
+  const Spinor<T> s = ev.lds(entry_of(d.op[0], pt));
+  const Vec4<T> V = ev.ldv(entry_of(d.op[1], pt));
+  ev.sts(d.out + v, ffv_row_prop(s, V, ev.ldm(d.mom), mt, ev.ip[d.prop]));
+} };
+MG_RC_TASK(K_COLPROP) {   // psi' = (qslash+m) Vslash psi / (q^2-m^2)
+  const Spinor<T> s = ev.lds(entry_of(d.op[0], pt));
+  const Vec4<T> V = ev.ldv(entry_of(d.op[1], pt));
+  ev.sts(d.out + v, ffv_col_prop(s, V, ev.ldm(d.mom), mt, ev.ip[d.prop]));
+} };
+MG_RC_TASK(K_FFCUR) {     // G = (psibar gamma^mu psi) / K^2
+  const Spinor<T> a = ev.lds(entry_of(d.op[0], pt));
+  const Spinor<T> b = ev.lds(entry_of(d.op[1], pt));
+  ev.stv(d.out + v, scale(ev.ip[d.prop], ff_current(a, b)));
+} };
+MG_RC_TASK(K_SLASHCOL) {  // half product Vslash psi (op0 = psi, op1 = V)
+  const Spinor<T> s = ev.lds(entry_of(d.op[0], pt));
+  const Vec4<T> V = ev.ldv(entry_of(d.op[1], pt));
+  ev.sts(d.out + v, slash_col(slash_parts(V), s));
+} };
+MG_RC_TASK(K_SLASHROW) {  // half product psibar Vslash (op0 = psibar, op1 = V)
+  const Spinor<T> s = ev.lds(entry_of(d.op[0], pt));
+  const Vec4<T> V = ev.ldv(entry_of(d.op[1], pt));
+  ev.sts(d.out + v, slash_row(slash_parts(V), s));
+} };
+#undef MG_RC_TASK
 
 // shared memory of one CTA
 template <class P, class T> struct Smem {
   typedef typename V2<T>::type W;
+  unsigned long long* pext4;   // [16]  nibble m of word v = pext(v, m)
   T* ext;   // [E][NPAR*4]   external momenta as loaded
   T* mom;   // [E][NMOM][4]
   T* ip;    // [E][NMOM]
   W* ent;   // [E][4][NSLOT]
   T* red;   // [NT/32]
+  static constexpr size_t kScalars = (size_t)P::E * (P::NPAR * 4 + P::NMOM * 5);
+  static constexpr size_t kEntOff = 128 + (kScalars * sizeof(T) + 15) / 16 * 16;
+  static constexpr size_t bytes() { return kEntOff + (size_t)P::E * 4 * P::NSLOT * sizeof(W) + (P::NT / 32) * sizeof(T) + 16; }
+  __device__ __forceinline__ void bind(unsigned char* raw) {
+    pext4 = reinterpret_cast<unsigned long long*>(raw);
+    ext = reinterpret_cast<T*>(raw + 128);
+    mom = ext + P::E * P::NPAR * 4;
+    ip = mom + P::E * P::NMOM * 4;
+    ent = reinterpret_cast<W*>(raw + kEntOff);
+    red = reinterpret_cast<T*>(ent + P::E * 4 * P::NSLOT);
+  }
   __device__ __forceinline__ View<T, P::NSLOT> view(int e) const {
     View<T, P::NSLOT> v;
-    v.mom = mom + e * P::NMOM * 4; v.ip = ip + e * P::NMOM; v.ent = ent + e * 4 * P::NSLOT;
+    v.ext = ext + e * P::NPAR * 4; v.mom = mom + e * P::NMOM * 4; v.ip = ip + e * P::NMOM; v.ent = ent + e * 4 * P::NSLOT;
     return v;
-  }
-  static constexpr size_t bytes() {
-    return ((size_t)P::E * (P::NPAR * 4 + P::NMOM * 5) * sizeof(T) + 15) / 16 * 16 + (size_t)P::E * 4 * P::NSLOT * sizeof(W) + (P::NT / 32) * sizeof(T) + 16;
   }
 };
 
@@ -179,8 +213,27 @@ template <class P, class T, int KIND, int NB> __device__ __forceinline__ void ru
   constexpr int PER = P::E << NB;
   const int fam = t / PER;
   if (fam >= nfam) return;
-  const int r = t - fam * PER;
-  Task<P, T, KIND>::run(P::node(first_node + fam), r & ((1 << NB) - 1), s.view(r >> NB), mt);
+  const int r = t - fam * PER, v = r & ((1 << NB) - 1);
+  Task<P, T, KIND>::run(P::node(first_node + fam), v, s.pext4[v], s.view(r >> NB), mt);
+}
+// line momenta (signed sums of external momenta) and inverse propagator denominators, in double also for
+// T = float (once per event; k_i.k_j cancels like theta^2 for collinear pairs, R19).  Task t = (event, entry).
+template <class P, class T> __device__ __forceinline__ void run_momtab(const Smem<P, T>& s, int t, T mt) {
+  if (t >= P::E * P::NMOM) return;
+  const int e = t / P::NMOM, m = t - e * P::NMOM;
+  const MomDef d = P::momdef(m);
+  double q[4] = {0, 0, 0, 0};
+#pragma unroll
+  for (int j = 0; j < P::NPAR; ++j) {
+    const double c = (double)d.c[j];
+#pragma unroll
+    for (int mu = 0; mu < 4; ++mu) q[mu] = fma(c, (double)s.ext[(e * P::NPAR + j) * 4 + mu], q[mu]);
+  }
+#pragma unroll
+  for (int mu = 0; mu < 4; ++mu) s.mom[(e * P::NMOM + m) * 4 + mu] = (T)q[mu];
+  double den = fma(q[0], q[0], fma(-q[1], q[1], fma(-q[2], q[2], -q[3] * q[3])));
+  if (d.propkind == 2) den = fma(-(double)mt, (double)mt, den);
+  s.ip[e * P::NMOM + m] = d.propkind ? (T)(1.0 / den) : (T)0;
 }
 
 // ---------------------------------------------------------------------------------------------------
@@ -191,13 +244,8 @@ __global__ void __launch_bounds__(P::NT, P::MINB) sigmakin_recycle_kernel(Consts
                                                                           T* __restrict__ me, const T* __restrict__ psw,
                                                                           T* __restrict__ evw, T* __restrict__ hel_out, uint64_t mask) {
   extern __shared__ __align__(16) unsigned char smem_raw[];
-  typedef typename V2<T>::type W;
   Smem<P, T> s;
-  s.ext = reinterpret_cast<T*>(smem_raw);
-  s.mom = s.ext + P::E * P::NPAR * 4;
-  s.ip = s.mom + P::E * P::NMOM * 4;
-  s.ent = reinterpret_cast<W*>(smem_raw + ((size_t)P::E * (P::NPAR * 4 + P::NMOM * 5) * sizeof(T) + 15) / 16 * 16);
-  s.red = reinterpret_cast<T*>(s.ent + P::E * 4 * P::NSLOT);
+  s.bind(smem_raw);
   const int tid = threadIdx.x;
   const int64_t ev0 = (int64_t)blockIdx.x * P::E;
 
@@ -208,24 +256,11 @@ __global__ void __launch_bounds__(P::NT, P::MINB) sigmakin_recycle_kernel(Consts
     if (ge >= n) ge = n - 1;
     s.ext[i] = __ldg(mom + (int64_t)r * ld + ge);
   }
-  __syncthreads();
-  // line momenta (signed sums of external momenta) and inverse propagator denominators, in double also
-  // for T = float (once per event; k_i.k_j cancels like theta^2 for collinear pairs, R19)
-  for (int i = tid; i < P::E * P::NMOM; i += P::NT) {
-    const int e = i / P::NMOM, m = i - e * P::NMOM;
-    const MomDef d = P::momdef(m);
-    double q[4] = {0, 0, 0, 0};
+  if (tid < 16) {
+    unsigned long long w = 0;
 #pragma unroll
-    for (int j = 0; j < P::NPAR; ++j) {
-      const double c = (double)d.c[j];
-#pragma unroll
-      for (int mu = 0; mu < 4; ++mu) q[mu] += c * (double)s.ext[(e * P::NPAR + j) * 4 + mu];
-    }
-#pragma unroll
-    for (int mu = 0; mu < 4; ++mu) s.mom[(e * P::NMOM + m) * 4 + mu] = (T)q[mu];
-    double den = fma(q[0], q[0], fma(-q[1], q[1], fma(-q[2], q[2], -q[3] * q[3])));
-    if (d.propkind == 2) den -= k.mt * k.mt;
-    s.ip[e * P::NMOM + m] = d.propkind ? (T)(1.0 / den) : (T)0;
+    for (int m = 0; m < 16; ++m) w |= (unsigned long long)pext(tid, m) << (4 * m);
+    s.pext4[tid] = w;
   }
   __syncthreads();
 

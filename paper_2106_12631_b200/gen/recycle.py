@@ -88,7 +88,7 @@ class Closure:
 
 
 class Program:
-    def __init__(self, ng, chunk_budget=300):
+    def __init__(self, ng, chunk_budget=200):
         self.ng = ng
         g = self.g = qcdgen.Generator(ng)
         self.npar = ng + 2
@@ -176,8 +176,10 @@ class Program:
                                 momA=self.kidx[a.subset], momB=self.kidx[b.subset]))
             else:
                 which, a, b, c = t[2], t[3], t[4], t[5]
-                out.append(dict(type=which, sign=t[0], ops=[self.nodes[a.name], self.nodes[b.name], self.nodes[c.name]],
-                                momA=0, momB=0))
+                ops = [self.nodes[a.name], self.nodes[b.name], self.nodes[c.name]]
+                # every structure is (X.Y) Z - (Z.Y) X after a permutation (csrc/recycle.cuh vvvv_acc)
+                cops = {1: [ops[0], ops[2], ops[1]], 2: ops, 3: [ops[1], ops[0], ops[2]]}[which]
+                out.append(dict(type=which, sign=t[0], ops=ops, cops=cops, momA=0, momB=0))
         return RNode(name, "VCUR", [self.gp[gi] for gi in subset], terms=out, prop=prop)
 
     # ------------------------------------------------------------------ closures as inner products
@@ -210,38 +212,69 @@ class Program:
 
     # ------------------------------------------------------------------ steps
     def _schedule(self, budget):
-        # levels of the base nodes
+        """Steps = producer steps ('P', nodes) and per-helicity chunks of closures ('F', closures).
+        Closures are chunked by the class (helicity bits, kind) of their half product, classes larger than
+        `budget` entries are split; every node is produced as late as possible (just before the first chunk
+        that needs it), which bounds the shared memory alive at once; independent producer steps are merged."""
         for n in self.nodes.values():
             n.level = 1 + max([o.level for o in n.operands()], default=-1)
-        nlev = 1 + max(n.level for n in self.nodes.values())
-        self.steps = []                                   # ('P', [nodes]) | ('F', [closures])
-        for lv in range(nlev):
-            self.steps.append(("P", [n for n in self.nodes.values() if n.level == lv]))
-        # chunks of closures: classes by (kind of new node, its number of helicity bits), small classes merged
+
         def new_node(c):
-            return c.a if c.a.name in self.half else (c.b if c.b.name in self.half else None)
+            return c.a if c.a.name in self.half else c.b
 
         classes = OrderedDict()
         for c in self.closures:
             nn = new_node(c)
-            classes.setdefault((nn.nbits, nn.kind), []).append(c)
+            classes.setdefault((nn.nbits, nn.kind), OrderedDict()).setdefault(nn.name, []).append(c)
         chunks, cur, cur_n = [], [], 0
         for key in sorted(classes):
-            cl = classes[key]
-            nnew = sum(n.nvar for n in {new_node(c).name: new_node(c) for c in cl}.values())
-            if cur and cur_n + nnew > budget:
+            names = list(classes[key])
+            total = sum(self.half[x].nvar for x in names)
+            if total > budget:                              # split a large class into equal parts
+                if cur:
+                    chunks.append(cur)
+                    cur, cur_n = [], 0
+                parts = -(-total // budget)
+                per = -(-len(names) // parts)
+                for i in range(0, len(names), per):
+                    chunks.append([c for x in names[i:i + per] for c in classes[key][x]])
+                continue
+            if cur and cur_n + total > budget:
                 chunks.append(cur)
                 cur, cur_n = [], 0
-            cur = cur + cl
-            cur_n += nnew
+            cur = cur + [c for x in names for c in classes[key][x]]
+            cur_n += total
         if cur:
             chunks.append(cur)
+        self.steps = []
+        done = set()
         for ch in chunks:
             hp = OrderedDict()
             for c in ch:
-                nn = new_node(c)
-                hp[nn.name] = nn
-            self.steps.append(("P", list(hp.values())))
+                hp[new_node(c).name] = new_node(c)
+            need, stack = OrderedDict(), []
+            for c in ch:
+                stack += [x for x in (c.a, c.b) if x.name not in self.half]
+            for n in hp.values():
+                stack += n.operands()
+            while stack:
+                x = stack.pop()
+                if x.name in done or x.name in need:
+                    continue
+                need[x.name] = x
+                stack += x.operands()
+            psteps = []
+            for lv in sorted({x.level for x in need.values()}):
+                psteps.append([x for x in self.nodes.values() if x.name in need and x.level == lv])
+            psteps.append(list(hp.values()))
+            done.update(need)
+            # merge a producer step into the previous one when it reads nothing born there
+            for ps in psteps:
+                prev = self.steps[-1] if self.steps and self.steps[-1][0] == "P" else None
+                if prev is not None and not any(o in prev[1] for x in ps for o in x.operands()):
+                    prev[1].extend(ps)
+                else:
+                    self.steps.append(("P", list(ps)))
             # closures sharing the second operand are adjacent: it is loaded once
             self.steps.append(("F", sorted(ch, key=lambda c: (c.b.name, c.a.name))))
         # birth / last use
@@ -256,8 +289,10 @@ class Program:
                     c.a.last = si
                     c.b.last = si
         self.all_nodes = [n for kind, items in self.steps if kind == "P" for n in items]
+        assert len(self.all_nodes) == len(self.nodes) + len(self.half)
         for n in self.all_nodes:
             assert n.last is not None and n.last > n.born, n.name
+            assert n.nbits <= 4, "the pext table of recycle.cuh covers 4 helicity bits per node"
             for o in n.operands():
                 assert o.born < n.born
 
@@ -304,7 +339,8 @@ class Program:
     def groups(nodes):
         gr = OrderedDict()
         for n in nodes:
-            gr.setdefault((n.kind, n.nbits), []).append(n)
+            kind = "EXT" if n.kind in ("POLVEC", "UBAR", "VSP") else n.kind     # externals share one divergent warp
+            gr.setdefault((kind, n.nbits), []).append(n)
         return gr
 
 
@@ -343,26 +379,33 @@ def emit(prog):
         w("  {{%s}, %d, 0},   // %s" % (", ".join(str(x) for x in c6), kind, nm))
     w("};")
     node_lines = []
+
+    def opw(consumer, x):
+        return "0x%08xu" % (x.slot | (4 * consumer.local_mask(x)) << 16)
+
     for n in order:
-        ops = [(0, 0), (0, 0)]
+        ops = ["0u", "0u"]
         aux, nterm = 0, 0
         if n.kind == "VCUR":
             aux, nterm = len(terms), len(n.params["terms"])
             for t in n.params["terms"]:
-                o = [(x.slot, n.local_mask(x)) for x in t["ops"]] + [(0, 0)] * (3 - len(t["ops"]))
-                terms.append("  {%d, %d, %d, %d, {%s}},   // %s: %s" % (t["type"], t["sign"], t["momA"], t["momB"],
-                             ", ".join("{%d, %d}" % x for x in o), n.name, " ".join(x.name for x in t["ops"])))
+                tops = t["ops"] if t["type"] == 0 else t["cops"]
+                o = [opw(n, x) for x in tops] + ["0u"] * (3 - len(tops))
+                terms.append("  {%d, %d, %d, 0, %s, {%s}},   // %s: %s" % (0 if t["type"] == 0 else 1, t["momA"], t["momB"],
+                             "0x80000000u" if t["sign"] < 0 else "0u", ", ".join(o), n.name, " ".join(x.name for x in tops)))
         else:
             for i, x in enumerate(n.ops):
-                ops[i] = (x.slot, n.local_mask(x))
+                ops[i] = opw(n, x)
             if n.kind == "POLVEC":
                 aux = 1 if n.params["outgoing"] else 0
+            elif n.kind in ("UBAR", "VSP"):
+                aux = 2 if n.kind == "UBAR" else 3
         prop = n.params.get("prop")
         node_lines.append("  {%d, %d, %d, %d, %d, {%s}},   // %d %s %s dep %s" % (
             n.slot, -1 if prop is None else prop, n.params.get("mom", 0), aux, nterm,
-            ", ".join("{%d, %d}" % x for x in ops), index[n.name], n.kind, n.name, "".join(map(str, n.dep))))
+            ", ".join(ops), index[n.name], n.kind, n.name, "".join(map(str, n.dep))))
     w("__constant__ rc::TermDesc kRcTerm_%s[%d] = {" % (tag, max(1, len(terms))))
-    for t in terms or ["  {0, 0, 0, 0, {{0, 0}, {0, 0}, {0, 0}}},"]:
+    for t in terms or ["  {0, 0, 0, 0, 0u, {0u, 0u, 0u}},"]:
         w(t)
     w("};")
     w("__constant__ rc::NodeDesc kRcNode_%s[%d] = {" % (tag, len(order)))
@@ -385,16 +428,23 @@ def emit(prog):
         if kind == "P":
             gr = Program.groups(items)
             bounds, b = [], 0
+            if si == 0:                                   # line momenta and propagators ride with the external wavefunctions
+                cnt = prog.E * len(prog.mom_defs)
+                bounds.append(("MOMTAB", 0, 0, 0, 0, (cnt + 31) // 32 * 32))
+                b = bounds[0][5]
             for (k, nb), ns in gr.items():
                 cnt = len(ns) * (prog.E << nb)
                 pad = (cnt + 31) // 32 * 32
                 bounds.append((k, nb, index[ns[0].name], len(ns), b, b + pad))
                 b += pad
-            w("    // step %d: %s" % (si, ", ".join("%d x %s/%d bits" % (len(ns), k, nb) for (k, nb), ns in gr.items())))
+            w("    // step %d: %s%s" % (si, "momentum table, " if si == 0 else "", ", ".join("%d x %s/%d bits" % (len(ns), k, nb) for (k, nb), ns in gr.items())))
             w("    for (int t = tid; t < %d; t += NT) {" % b)
             for i, (k, nb, first, nfam, lo, hi) in enumerate(bounds):
                 cond = "" if len(bounds) == 1 else ("if (t < %d) " % hi if i == 0 else ("else if (t < %d) " % hi if i < len(bounds) - 1 else "else "))
-                w("      %src::run_group<%s, T, rc::K_%s, %d>(s, %d, %d, t - %d, mt);" % (cond, name, k, nb, first, nfam, lo))
+                if k == "MOMTAB":
+                    w("      %src::run_momtab<%s, T>(s, t, mt);" % (cond, name))
+                else:
+                    w("      %src::run_group<%s, T, rc::K_%s, %d>(s, %d, %d, t - %d, mt);" % (cond, name, k, nb, first, nfam, lo))
             w("    }")
             w("    __syncthreads();")
         else:
