@@ -93,7 +93,9 @@ class Program:
         g = self.g = qcdgen.Generator(ng)
         self.npar = ng + 2
         self.nhel = 1 << self.npar
-        self.E = max(1, 128 // self.nhel)
+        # events per CTA and resident CTAs per SM: tuned on B200; the environment overrides are for sweeps
+        self.E = int(os.environ.get('MG_RC_E', 3 if ng == 4 else max(1, 128 // self.nhel)))
+        self.MINB = int(os.environ.get('MG_RC_MINB', 2 if ng == 4 else 3))
         self.NT = self.E * self.nhel
         self.gp = g.gl_particle
         self._build_momenta()
@@ -413,7 +415,7 @@ def emit(prog):
         w(l)
     w("};")
     w("struct %s {" % name)
-    w("  static constexpr int NPAR = %d, NHEL = %d, NFLOW = %d, E = %d, NT = %d, MINB = %d;" % (npar, prog.nhel, nf, prog.E, prog.NT, 3))
+    w("  static constexpr int NPAR = %d, NHEL = %d, NFLOW = %d, E = %d, NT = %d, MINB = %d;" % (npar, prog.nhel, nf, prog.E, prog.NT, prog.MINB))
     w("  static constexpr int NMOM = %d, NSLOT = %d;" % (len(prog.mom_defs), prog.nslot))
     w("  static __device__ __forceinline__ const rc::NodeDesc& node(int i) { return kRcNode_%s[i]; }" % tag)
     w("  static __device__ __forceinline__ const rc::TermDesc& term(int i) { return kRcTerm_%s[i]; }" % tag)
