@@ -270,6 +270,10 @@ def main():
         out["clocks"] = sampler.result()
         try:
             out["roofline"]["measured_fma_chain_tflops"] = mg.measure_alu_peak(prec, local_rank)
+            # how the FMA is fed decides its rate on sm_100a: three distinct register operands vs tensor-core FP64
+            out["roofline"]["measured_fma_3reg_tflops"] = mg.measure_alu_mode(prec, local_rank, 1)
+            if prec == 0:
+                out["roofline"]["measured_dmma_tflops"] = mg.measure_alu_mode(prec, local_rank, 2)
         except Exception as e:
             out["roofline"]["measured_fma_chain_tflops"] = "failed: %s" % e
         tr = os.path.join(ROOT, "profiles", "traffic.json")

@@ -146,6 +146,12 @@ double mg_last_kernel_ms(const mg_process* p);
  * register-only chain microbenchmark (the denominator of the "alu" roofline).
  * Synchronous, takes ~0.1 s. */
 int mg_measure_alu_peak(int precision, int device, double* h_tflops_out);
+/* The same measurement for the three ways an FMA can be fed on sm_100a (SURVEY.md §8(d) asks for
+ * the peak to be confirmed on the box): mode 0 = the chain of mg_measure_alu_peak (one register operand plus two
+ * loop constants), mode 1 = three distinct register operands per FMA (what a product of two loaded wavefunctions
+ * accumulates into), mode 2 = the FP64 tensor-core instruction mma.sync m8n8k4 (FP64 only, else MG_EINVAL).
+ * Synchronous, ~0.1 s.  Errors as mg_measure_alu_peak. */
+int mg_measure_alu_mode(int precision, int device, int mode, double* h_tflops_out);
 
 const char* mg_strerror(int code);
 const char* mg_version(void);

@@ -67,6 +67,7 @@ def lib():
         "mg_bytes_per_event": (i64, [vp, C.c_int]),
         "mg_last_kernel_ms": (C.c_double, [vp]),
         "mg_measure_alu_peak": (C.c_int, [C.c_int, C.c_int, C.POINTER(C.c_double)]),
+        "mg_measure_alu_mode": (C.c_int, [C.c_int, C.c_int, C.c_int, C.POINTER(C.c_double)]),
         "mg_strerror": (C.c_char_p, [C.c_int]),
         "mg_version": (C.c_char_p, []),
     }
@@ -82,7 +83,7 @@ EXPORTED = ["mg_default_params", "mg_init_process", "mg_free_process", "mg_n_ext
             "mg_padded_stride", "mg_rng_words", "mg_rng", "mg_rambo", "mg_generate", "mg_filter_helicities",
             "mg_set_helicity_mask", "mg_get_helicity_mask", "mg_sigmakin", "mg_sigmakin_per_helicity",
             "mg_sigmakin_host", "mg_run_host", "mg_flops_per_event", "mg_bytes_per_event", "mg_last_kernel_ms",
-            "mg_measure_alu_peak", "mg_strerror", "mg_version"]
+            "mg_measure_alu_peak", "mg_measure_alu_mode", "mg_strerror", "mg_version"]
 
 
 def _check(rc):
@@ -101,6 +102,13 @@ def default_params(process, precision=FP64, device=0, **kw):
     for k, v in kw.items():
         setattr(p, k, v)
     return p
+
+
+def measure_alu_mode(precision=FP64, device=0, mode=0):
+    """TFLOP/s of mg_measure_alu_mode: 0 = FMA chain, 1 = three distinct register operands, 2 = FP64 mma.sync m8n8k4."""
+    v = C.c_double()
+    _check(lib().mg_measure_alu_mode(precision, device, mode, C.byref(v)))
+    return v.value
 
 
 def measure_alu_peak(precision=FP64, device=0):

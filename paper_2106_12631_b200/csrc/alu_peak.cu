@@ -28,6 +28,73 @@ __global__ void __launch_bounds__(256) fma_chain_kernel(T a, T b, int iters, T* 
   if (s == (T)123456789) out[0] = s;  // never true; keeps the chains alive
 }
 
+// mode 1: every FMA reads THREE distinct registers (what products of two loaded operands accumulate into).
+// On B200 the FP64 FMA then issues once per 3 cycles instead of 2 (three 64-bit operands through a two-bank
+// register file; the operand-reuse cache and constant operands avoid it) — DESIGN.md §6.
+template <class T, int N>
+__global__ void __launch_bounds__(256) fma3_kernel(int iters, T* __restrict__ out) {
+  T x[N];
+#pragma unroll
+  for (int i = 0; i < N; ++i) x[i] = (T)1 + (T)(threadIdx.x + i) * (T)1e-9;
+#pragma unroll 1
+  for (int it = 0; it < iters; ++it) {
+#pragma unroll
+    for (int i = 0; i < N; ++i) x[i] = fma_t<T>(x[(i + 5) % N], x[(i + 11) % N], x[i]);
+  }
+  T s = 0;
+#pragma unroll
+  for (int i = 0; i < N; ++i) s += x[i];
+  if (s == (T)123456789) out[0] = s;
+}
+
+// mode 2: FP64 tensor-core path, mma.sync m8n8k4 (DMMA): 256 FMA per warp instruction, 8 independent accumulators
+__global__ void __launch_bounds__(256) dmma_kernel(int iters, double* __restrict__ out) {
+  double c[16];
+#pragma unroll
+  for (int i = 0; i < 16; ++i) c[i] = threadIdx.x * 1e-4 + i;
+  const double a = 1.0000001, b = 0.5;
+#pragma unroll 1
+  for (int it = 0; it < iters; ++it) {
+#pragma unroll
+    for (int i = 0; i < 8; ++i)
+      asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};" : "+d"(c[2 * i]), "+d"(c[2 * i + 1]) : "d"(a), "d"(b));
+  }
+  double s = 0;
+#pragma unroll
+  for (int i = 0; i < 16; ++i) s += c[i];
+  if (s == 123456789.0) out[0] = s;
+}
+
+template <class T>
+cudaError_t run_mode(int sm_count, int mode, double* tflops) {
+  const int blocks = sm_count * 8, threads = 256, iters = 4096;
+  T* d = nullptr;
+  cudaError_t e = cudaMalloc(&d, sizeof(T));
+  if (e != cudaSuccess) return e;
+  cudaEvent_t e0, e1;
+  cudaEventCreate(&e0); cudaEventCreate(&e1);
+  double best = 0;
+  for (int rep = 0; rep < 4; ++rep) {
+    cudaEventRecord(e0);
+    double flops;
+    if (mode == 1) {
+      fma3_kernel<T, 24><<<blocks, threads>>>(iters, d);
+      flops = 2.0 * 24 * iters * (double)blocks * threads;
+    } else {
+      dmma_kernel<<<blocks, threads>>>(iters, reinterpret_cast<double*>(d));
+      flops = 2.0 * 8 * 8 * 4 * 8.0 * iters * (double)blocks * threads / 32;
+    }
+    cudaEventRecord(e1);
+    e = cudaEventSynchronize(e1);
+    if (e != cudaSuccess) break;
+    float ms = 0; cudaEventElapsedTime(&ms, e0, e1);
+    if (rep > 0 && ms > 0) best = fmax(best, flops / (ms * 1e-3) * 1e-12);
+  }
+  cudaEventDestroy(e0); cudaEventDestroy(e1); cudaFree(d);
+  *tflops = best;
+  return e == cudaSuccess ? cudaGetLastError() : e;
+}
+
 template <class T>
 cudaError_t run(int sm_count, double* tflops) {
   constexpr int CHAINS = 16;
@@ -55,10 +122,12 @@ cudaError_t run(int sm_count, double* tflops) {
 
 }  // namespace
 
-cudaError_t measure_alu_peak(int precision, int device, double* tflops) {
+cudaError_t measure_alu_peak(int precision, int device, int mode, double* tflops) {
   cudaDeviceProp prop;
   cudaError_t e = cudaGetDeviceProperties(&prop, device);
   if (e != cudaSuccess) return e;
+  if (mode == 1) return precision == MG_FP64 ? run_mode<double>(prop.multiProcessorCount, 1, tflops) : run_mode<float>(prop.multiProcessorCount, 1, tflops);
+  if (mode == 2) return run_mode<double>(prop.multiProcessorCount, 2, tflops);
   return precision == MG_FP64 ? run<double>(prop.multiProcessorCount, tflops) : run<float>(prop.multiProcessorCount, tflops);
 }
 

@@ -345,7 +345,16 @@ int mg_measure_alu_peak(int precision, int device, double* h_tflops_out) {
   int ndev = 0;
   if (cudaGetDeviceCount(&ndev) != cudaSuccess || device >= ndev) { cudaGetLastError(); return MG_ECUDA; }
   DeviceGuard g(device); if (!g.ok) return MG_ECUDA;
-  return cuda_rc(measure_alu_peak(precision, device, h_tflops_out));
+  return cuda_rc(measure_alu_peak(precision, device, 0, h_tflops_out));
+}
+
+int mg_measure_alu_mode(int precision, int device, int mode, double* h_tflops_out) {
+  if (!h_tflops_out || device < 0 || (precision != MG_FP64 && precision != MG_FP32) || mode < 0 || mode > 2) return MG_EINVAL;
+  if (mode == 2 && precision != MG_FP64) return MG_EINVAL;
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || device >= ndev) { cudaGetLastError(); return MG_ECUDA; }
+  DeviceGuard g(device); if (!g.ok) return MG_ECUDA;
+  return cuda_rc(measure_alu_peak(precision, device, mode, h_tflops_out));
 }
 
 double mg_last_kernel_ms(const mg_process* p) { return p ? p->last_kernel_ms : 0.0; }

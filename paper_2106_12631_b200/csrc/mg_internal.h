@@ -28,7 +28,7 @@ struct mg_process {
 namespace mg {
 
 // alu_peak.cu
-cudaError_t measure_alu_peak(int precision, int device, double* tflops);
+cudaError_t measure_alu_peak(int precision, int device, int mode, double* tflops);
 
 // rng_rambo.cu
 cudaError_t launch_rng_words(const mg_process* p, uint64_t seed, uint64_t first, int64_t n, int64_t ld,

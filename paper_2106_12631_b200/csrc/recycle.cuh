@@ -240,7 +240,7 @@ template <class P, class T> __device__ __forceinline__ void run_momtab(const Sme
 // the kernel: grid = ceil(n / E) CTAs of NT = E * NHEL threads
 // ---------------------------------------------------------------------------------------------------
 template <class P, class T, bool PER_HEL>
-__global__ void __launch_bounds__(P::NT, P::MINB) sigmakin_recycle_kernel(Consts k, const T* __restrict__ mom, int64_t n, int64_t ld,
+__global__ void __launch_bounds__(P::NT, sizeof(T) == 8 ? P::MINB : P::MINB32) sigmakin_recycle_kernel(Consts k, const T* __restrict__ mom, int64_t n, int64_t ld,
                                                                           T* __restrict__ me, const T* __restrict__ psw,
                                                                           T* __restrict__ evw, T* __restrict__ hel_out, uint64_t mask) {
   extern __shared__ __align__(16) unsigned char smem_raw[];

@@ -94,8 +94,9 @@ class Program:
         self.npar = ng + 2
         self.nhel = 1 << self.npar
         # events per CTA and resident CTAs per SM: tuned on B200; the environment overrides are for sweeps
-        self.E = int(os.environ.get('MG_RC_E', 3 if ng == 4 else max(1, 128 // self.nhel)))
+        self.E = int(os.environ.get('MG_RC_E', 4 if ng == 4 else max(1, 128 // self.nhel)))
         self.MINB = int(os.environ.get('MG_RC_MINB', 2 if ng == 4 else 3))
+        self.MINB32 = int(os.environ.get('MG_RC_MINB32', 3 if ng == 4 else self.MINB))      # FP32: half the registers and shared memory
         self.NT = self.E * self.nhel
         self.gp = g.gl_particle
         self._build_momenta()
@@ -415,7 +416,7 @@ def emit(prog):
         w(l)
     w("};")
     w("struct %s {" % name)
-    w("  static constexpr int NPAR = %d, NHEL = %d, NFLOW = %d, E = %d, NT = %d, MINB = %d;" % (npar, prog.nhel, nf, prog.E, prog.NT, prog.MINB))
+    w("  static constexpr int NPAR = %d, NHEL = %d, NFLOW = %d, E = %d, NT = %d, MINB = %d, MINB32 = %d;" % (npar, prog.nhel, nf, prog.E, prog.NT, prog.MINB, prog.MINB32))
     w("  static constexpr int NMOM = %d, NSLOT = %d;" % (len(prog.mom_defs), prog.nslot))
     w("  static __device__ __forceinline__ const rc::NodeDesc& node(int i) { return kRcNode_%s[i]; }" % tag)
     w("  static __device__ __forceinline__ const rc::TermDesc& term(int i) { return kRcTerm_%s[i]; }" % tag)
