@@ -15,6 +15,15 @@ template <> MG_HD float fma_<float>(float a, float b, float c) { return fmaf(a, 
 template <class T> MG_HD T sqrt_(T a);
 template <> MG_HD double sqrt_<double>(double a) { return sqrt(a); }
 template <> MG_HD float sqrt_<float>(float a) { return sqrtf(a); }
+// 1/sqrt(a) in one step (one MUFU.RSQ seed + Newton instead of a square root followed by a division)
+template <class T> MG_HD T rsqrt_(T a);
+#ifdef __CUDA_ARCH__
+template <> MG_HD double rsqrt_<double>(double a) { return rsqrt(a); }
+template <> MG_HD float rsqrt_<float>(float a) { return rsqrtf(a); }
+#else
+template <> MG_HD double rsqrt_<double>(double a) { return 1.0 / sqrt(a); }
+template <> MG_HD float rsqrt_<float>(float a) { return 1.0f / sqrtf(a); }
+#endif
 template <class T> MG_HD T abs_(T a) { return a < (T)0 ? -a : a; }
 
 template <class T> struct cx {

@@ -20,7 +20,37 @@ namespace mg {
 struct Eemumu {
   static constexpr int NHEL = 16;
   static constexpr int NPAR = 4;
-  template <class T> struct Event { Mom<T> p[4]; Mom<T> q; T is; cx<T> bw; };
+  // Massless helicity spinors need three reals per particle (the "simplified" IXXXXX/OXXXXX of PAPER.md:136):
+  //   omega_+ chi_+ = (a, b),  omega_+ chi_- = (-b^*, a),   a = sqrt(P+pz),  b = (px + i py)/sqrt(P+pz),
+  // P+pz evaluated as pT^2/(P-pz) for pz < 0 (R19); along -z: a = 0, b = sqrt(2P) (B1).  One square root, one
+  // reciprocal square root and at most one division per particle and event, shared by all 16 helicity combinations.
+  template <class T> struct Event { Mom<T> p[4]; Mom<T> q; T is; cx<T> bw; T a[4]; cx<T> b[4]; };
+
+  template <class T> static MG_HD void massless_frame(Mom<T> p, T& a, cx<T>& b) {
+    const T px = p.v[1], py = p.v[2], pz = p.v[3];
+    const T pt2 = fma_<T>(px, px, py * py);
+    const T P = sqrt_<T>(fma_<T>(pz, pz, pt2));
+    if (pt2 == (T)0 && pz < (T)0) { a = (T)0; b = cx<T>(sqrt_<T>(P + P), (T)0); return; }
+    const T Ppz = (pz >= (T)0) ? (P + pz) : pt2 / (P - pz);
+    const T r = rsqrt_<T>(Ppz);
+    a = Ppz * r;
+    b = cx<T>(px * r, py * r);
+  }
+  // u(p, l): incoming fermion; v(p, l): outgoing antifermion (helas.cuh spinor_u / spinor_v at m = 0)
+  template <class T> static MG_HD Spinor<T> u0(T a, cx<T> b, int l) {
+    Spinor<T> s;
+    const cx<T> z((T)0, (T)0);
+    if (l > 0) { s.l[0] = z; s.l[1] = z; s.r[0] = cx<T>(a, (T)0); s.r[1] = b; }
+    else { s.l[0] = cx<T>(-b.re, b.im); s.l[1] = cx<T>(a, (T)0); s.r[0] = z; s.r[1] = z; }
+    return s;
+  }
+  template <class T> static MG_HD Spinor<T> v0(T a, cx<T> b, int l) {
+    Spinor<T> s;
+    const cx<T> z((T)0, (T)0);
+    if (l > 0) { s.l[0] = cx<T>(-b.re, b.im); s.l[1] = cx<T>(a, (T)0); s.r[0] = z; s.r[1] = z; }
+    else { s.l[0] = z; s.l[1] = z; s.r[0] = cx<T>(-a, (T)0); s.r[1] = -b; }
+    return s;
+  }
 
   template <class T> static MG_HD void finish(Event<T>& ev, const Consts& k) {
     ev.q = ev.p[0] + ev.p[1];
@@ -30,15 +60,17 @@ struct Eemumu {
     const T dr = s - (T)k.mZ2, di = (T)k.mZgZ;
     const T inv = (T)1 / fma_<T>(dr, dr, di * di);
     ev.bw = cx<T>(dr * inv, -di * inv);
+#pragma unroll
+    for (int i = 0; i < 4; ++i) massless_frame<T>(ev.p[i], ev.a[i], ev.b[i]);
   }
 
   template <class T> static MG_HD T helicity(const Event<T>& ev, int ihel, const Consts& k) {
     const int h0 = (ihel & 1) ? 1 : -1, h1 = (ihel & 2) ? 1 : -1, h2 = (ihel & 4) ? 1 : -1, h3 = (ihel & 8) ? 1 : -1;
     // OXXXXX / IXXXXX: incoming e+ -> vbar, incoming e- -> u, outgoing mu+ -> v, outgoing mu- -> ubar
-    const Spinor<T> vbar_ep = bar(spinor_v<T>(ev.p[0], (T)0, h0));
-    const Spinor<T> u_em = spinor_u<T>(ev.p[1], (T)0, h1);
-    const Spinor<T> v_mup = spinor_v<T>(ev.p[2], (T)0, h2);
-    const Spinor<T> ubar_mum = bar(spinor_u<T>(ev.p[3], (T)0, h3));
+    const Spinor<T> vbar_ep = bar(v0<T>(ev.a[0], ev.b[0], h0));
+    const Spinor<T> u_em = u0<T>(ev.a[1], ev.b[1], h1);
+    const Spinor<T> v_mup = v0<T>(ev.a[2], ev.b[2], h2);
+    const Spinor<T> ubar_mum = bar(u0<T>(ev.a[3], ev.b[3], h3));
     const T e = (T)k.ee, gzl = (T)k.gzl, gzr = (T)k.gzr;
 
     // chirality-split current of the electron line: J_R = a sigma^mu psi_R, J_L = b sigmabar^mu psi_L

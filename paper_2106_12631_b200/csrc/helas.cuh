@@ -70,7 +70,7 @@ template <class T> MG_HD Chi<T> chi(Mom<T> p, T P, int lambda) {
     return x;
   }
   const T Ppz = (pz >= (T)0) ? (P + pz) : pt2 / (P - pz);
-  const T nrm = (T)1 / sqrt_<T>((T)2 * P * Ppz);
+  const T nrm = rsqrt_<T>((T)2 * P * Ppz);
   if (lambda > 0) { x.c[0] = cx<T>(Ppz * nrm, (T)0); x.c[1] = cx<T>(px * nrm, py * nrm); }
   else            { x.c[0] = cx<T>(-px * nrm, py * nrm); x.c[1] = cx<T>(Ppz * nrm, (T)0); }
   return x;
@@ -84,8 +84,9 @@ template <class T> MG_HD Chi<T> chi(Mom<T> p, T P, int lambda) {
 // ubar, vbar = psi^dagger gamma^0 = (psi_R^dagger | psi_L^dagger)   outgoing fermion / incoming antifermion (OXXXXX)
 template <class T> MG_HD Spinor<T> spinor_u(Mom<T> p, T m, int lambda) {
   const T P = sqrt_<T>(fma_<T>(p.v[1], p.v[1], fma_<T>(p.v[2], p.v[2], p.v[3] * p.v[3])));
-  const T wp = sqrt_<T>((m == (T)0 ? P : p.v[0]) + P);
-  const T wm = m / wp;
+  const T ep = (m == (T)0 ? P : p.v[0]) + P;
+  const T iw = rsqrt_<T>(ep);
+  const T wp = ep * iw, wm = m * iw;
   const Chi<T> x = chi<T>(p, P, lambda);
   const T wl = lambda > 0 ? wm : wp, wr = lambda > 0 ? wp : wm;
   Spinor<T> s;
@@ -95,8 +96,9 @@ template <class T> MG_HD Spinor<T> spinor_u(Mom<T> p, T m, int lambda) {
 }
 template <class T> MG_HD Spinor<T> spinor_v(Mom<T> p, T m, int lambda) {
   const T P = sqrt_<T>(fma_<T>(p.v[1], p.v[1], fma_<T>(p.v[2], p.v[2], p.v[3] * p.v[3])));
-  const T wp = sqrt_<T>((m == (T)0 ? P : p.v[0]) + P);
-  const T wm = m / wp;
+  const T ep = (m == (T)0 ? P : p.v[0]) + P;
+  const T iw = rsqrt_<T>(ep);
+  const T wp = ep * iw, wm = m * iw;
   const Chi<T> x = chi<T>(p, P, -lambda);
   const T wl = lambda > 0 ? wp : wm, wr = lambda > 0 ? -wm : -wp;
   Spinor<T> s;
@@ -130,8 +132,8 @@ template <class T> MG_HD Vec4<T> polvec(Mom<T> p, int lambda, bool outgoing) {
     e.v[3] = cx<T>((T)0, (T)0);
     return e;
   }
-  const T ipt = (T)1 / sqrt_<T>(pt2);
-  const T iP = (T)1 / sqrt_<T>(fma_<T>(pz, pz, pt2));
+  const T ipt = rsqrt_<T>(pt2);
+  const T iP = rsqrt_<T>(fma_<T>(pz, pz, pt2));
   const T ct = pz * iP, st = pt2 * ipt * iP, cp = px * ipt, sp = py * ipt;
   e.v[1] = cx<T>(-l * ct * cp * r2, cj * sp * r2);
   e.v[2] = cx<T>(-l * ct * sp * r2, -cj * cp * r2);
