@@ -93,10 +93,12 @@ class Program:
         g = self.g = qcdgen.Generator(ng)
         self.npar = ng + 2
         self.nhel = 1 << self.npar
-        # events per CTA and resident CTAs per SM: tuned on B200; the environment overrides are for sweeps
-        self.E = int(os.environ.get('MG_RC_E', 4 if ng == 4 else max(1, 128 // self.nhel)))
-        self.MINB = int(os.environ.get('MG_RC_MINB', 2 if ng == 4 else 3))
-        self.MINB32 = int(os.environ.get('MG_RC_MINB32', 3 if ng == 4 else self.MINB))      # FP32: half the registers and shared memory
+        # events per CTA and resident CTAs per SM (FP64 / FP32): tuned on B200 (profiles/r01_c_*); the
+        # environment overrides MG_RC<ng>_E / _MINB / _MINB32 are for sweeps
+        dflt = {2: (8, 3, 3), 3: (4, 4, 5), 4: (4, 2, 3)}[ng]
+        self.E = int(os.environ.get('MG_RC%d_E' % ng, dflt[0]))
+        self.MINB = int(os.environ.get('MG_RC%d_MINB' % ng, dflt[1]))
+        self.MINB32 = int(os.environ.get('MG_RC%d_MINB32' % ng, dflt[2]))
         self.NT = self.E * self.nhel
         self.gp = g.gl_particle
         self._build_momenta()
