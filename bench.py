@@ -187,6 +187,41 @@ def time_workload(mg, torch, name, device_index, steps, warmup, dist=None, sampl
             "seed": seed, "cfg": cfg, "world": world}
 
 
+def stage_rates(mg, torch, r, reps=20):
+    """A1-A4 alone: HBM GB/s of the RNG, RAMBO and fused generate kernels (north_star: "HBM GB/s for the RNG and RAMBO
+    stages"), algorithmic bytes of mg_bytes_per_event over the mean launch time, against MEASURED_PEAKS.json hbm_gbs."""
+    P, n, ld = r["P"], r["n"], r["ld"]
+    rnd = P.empty(4 * P.n_final, n, ld)
+    mom = P.empty(4 * P.n_external, n, ld)
+    w = torch.empty(ld, dtype=P.dtype, device=P.device)
+    hbm = measured_peaks().get("hbm_gbs")
+    calls = {"rng": (lambda i: P.rng(r["seed"], i * n, n, out=rnd), mg.STAGE_RNG),
+             "rambo": (lambda i: P.rambo(rnd, n, mom, w), mg.STAGE_RAMBO),
+             "generate": (lambda i: P.generate(r["seed"], i * n, n, mom, w), mg.STAGE_GENERATE)}
+    me = torch.empty(ld, dtype=P.dtype, device=P.device)
+    ew = torch.empty(ld, dtype=P.dtype, device=P.device)
+    # A1-A13 in one call, momenta never stored: whole-path MEs/s next to the three-kernel step
+    calls["fused_path"] = (lambda i: P.sigmakin_fused(r["seed"], i * n, n, me, w, ew), None)
+    out = {}
+    for name, (fn, stage) in calls.items():
+        for i in range(3):
+            fn(i)
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        a.record()
+        for i in range(reps):
+            fn(i)
+        b.record()
+        torch.cuda.synchronize()
+        ms = a.elapsed_time(b) / reps
+        if stage is None:
+            out[name] = {"ms": ms, "MEs_per_s": n / (ms * 1e-3)}
+            continue
+        gbs = n * P.bytes_per_event(stage) / (ms * 1e-3) / 1e9
+        out[name] = {"ms": ms, "GB/s": gbs, "frac_hbm": gbs / hbm if hbm else None, "events_per_s": n / (ms * 1e-3)}
+    return out
+
+
 def e2e_measure(mg, torch, r, steps):
     """End to end through the C ABI with HOST buffers: momenta H2D, sigmaKin, ME D2H (mg_sigmakin_host)."""
     P, n, ld = r["P"], r["n"], r["ld"]
@@ -276,6 +311,10 @@ def main():
                 out["roofline"]["measured_dmma_tflops"] = mg.measure_alu_mode(prec, local_rank, 2)
         except Exception as e:
             out["roofline"]["measured_fma_chain_tflops"] = "failed: %s" % e
+        try:
+            out["stages"] = stage_rates(mg, torch, r)
+        except Exception as e:
+            out["stages"] = "failed: %s" % e
         tr = os.path.join(ROOT, "profiles", "traffic.json")
         if os.path.exists(tr):
             out["roofline"]["traffic"] = json.load(open(tr)).get(args.workload)
@@ -292,7 +331,7 @@ def main():
                 others.append({"workload": name, "value": o["n"] * 3 / (o["total_ms"] * 1e-3), "unit": "MEs/s",
                                "sigmakin_MEs_per_s": o["n"] / (o["kern_ms"] * 1e-3), "sigmakin_ms": o["kern_ms"],
                                "alu_frac": tf / pk, "flops_per_event": o["flops_per_event"], "mean_me": o["mean_me"],
-                               "all_finite": o["finite"]})
+                               "all_finite": o["finite"], "stages": stage_rates(mg, torch, o, reps=10)})
                 del o
                 torch.cuda.empty_cache()
             except Exception as e:

@@ -102,6 +102,16 @@ int mg_rambo(mg_process* p, const void* d_rnd, int64_t n, int64_t ld,
 int mg_generate(mg_process* p, uint64_t seed, uint64_t first_event, int64_t n, int64_t ld,
                 void* d_momenta, void* d_ps_weight, void* stream);
 
+/* A1-A13 fused (PAPER.md:112-118 copy:compute balance): random numbers, momenta and matrix
+ * element of events first_event .. first_event+n-1 without the momenta ever being stored.  Writes me[n] and, if
+ * non-NULL, ps_weight[n] and event_weight[n] = ps_weight * me (R18); uses the installed helicity mask.  e+e- ->
+ * mu+mu- and g g -> t t~ run one kernel with everything in registers; the shared-memory kernels of g g -> t t~ g(g)
+ * stage the momenta in a device scratch buffer owned by the handle (grown on first use: that call synchronises the
+ * device; later calls are asynchronous on `stream`).  Same values as mg_generate + mg_sigmakin up to rounding of
+ * contracted multiply-adds.  Errors: MG_EINVAL (NULL/misaligned d_me, bad handle, n < 0), MG_ENOMEM, MG_ECUDA. */
+int mg_sigmakin_fused(mg_process* p, uint64_t seed, uint64_t first_event, int64_t n,
+                      void* d_me, void* d_ps_weight, void* d_event_weight, void* stream);
+
 /* A12: good-helicity filter (R16).  Evaluates every helicity combination on the
  * first probe_n events of d_momenta (1 <= probe_n <= n... the caller guarantees probe_n events are
  * present), marks h good iff max_e |M|^2_h / sum_h' |M|^2_h' > 1e-10, returns the mask in

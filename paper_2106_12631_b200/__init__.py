@@ -61,6 +61,7 @@ def lib():
         "mg_get_helicity_mask": (C.c_int, [vp, C.POINTER(u64)]),
         "mg_sigmakin": (C.c_int, [vp, vp, i64, i64, vp, vp, vp, vp]),
         "mg_sigmakin_per_helicity": (C.c_int, [vp, vp, i64, i64, vp, vp]),
+        "mg_sigmakin_fused": (C.c_int, [vp, u64, u64, i64, vp, vp, vp, vp]),
         "mg_sigmakin_host": (C.c_int, [vp, vp, i64, i64, vp]),
         "mg_run_host": (C.c_int, [vp, u64, u64, i64, i64, vp, vp, vp]),
         "mg_flops_per_event": (i64, [vp, C.c_int]),
@@ -81,7 +82,7 @@ def lib():
 EXPORTED = ["mg_default_params", "mg_init_process", "mg_free_process", "mg_n_external", "mg_n_final", "mg_n_helicities",
             "mg_n_colour_flows", "mg_n_diagrams", "mg_n_amplitudes", "mg_me_denominator", "mg_colour_matrix",
             "mg_padded_stride", "mg_rng_words", "mg_rng", "mg_rambo", "mg_generate", "mg_filter_helicities",
-            "mg_set_helicity_mask", "mg_get_helicity_mask", "mg_sigmakin", "mg_sigmakin_per_helicity",
+            "mg_set_helicity_mask", "mg_get_helicity_mask", "mg_sigmakin", "mg_sigmakin_per_helicity", "mg_sigmakin_fused",
             "mg_sigmakin_host", "mg_run_host", "mg_flops_per_event", "mg_bytes_per_event", "mg_last_kernel_ms",
             "mg_measure_alu_peak", "mg_measure_alu_mode", "mg_strerror", "mg_version"]
 
@@ -212,6 +213,14 @@ class Process:
         out = out if out is not None else self.empty(self.n_helicities, n, ld)
         _check(lib().mg_sigmakin_per_helicity(self._h, _ptr(momenta), n, ld, _ptr(out), _stream(self.device)))
         return out
+
+    def sigmakin_fused(self, seed, first_event, n, me=None, ps_weight=None, event_weight=None):
+        """mg_sigmakin_fused: random numbers -> momenta -> matrix element in one pass, momenta never stored."""
+        me = me if me is not None else torch.empty(n, dtype=self.dtype, device=self.device)
+        _check(lib().mg_sigmakin_fused(self._h, seed, first_event, n, _ptr(me),
+                                       _ptr(ps_weight) if ps_weight is not None else None,
+                                       _ptr(event_weight) if event_weight is not None else None, _stream(self.device)))
+        return me
 
     # ---- host-buffer (end-to-end) forms; tensors are CPU tensors (pinned for speed)
     def sigmakin_host(self, h_momenta, n, h_me):

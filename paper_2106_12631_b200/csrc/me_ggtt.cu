@@ -13,3 +13,10 @@ namespace mg {
 cudaError_t launch_me_ggtt(const mg_process* p, const MeArgs& a, cudaStream_t s) { return launch_sigmakin<Ggtt>(p, a, s); }
 }  // namespace mg
 #endif
+#include "gen_ggtt.cuh"
+#include "fused.cuh"
+namespace mg {
+cudaError_t launch_fused_ggtt(const mg_process* p, uint64_t seed, uint64_t first, int64_t n, void* me, void* psw, void* evw, cudaStream_t s) {
+  return launch_fused<Ggtt, 2, true>(p, seed, first, n, me, psw, evw, s);
+}
+}  // namespace mg

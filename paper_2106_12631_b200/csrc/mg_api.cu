@@ -204,6 +204,28 @@ int mg_sigmakin(mg_process* p, const void* d_momenta, int64_t n, int64_t ld, voi
   return cuda_rc(launch_me(p, a, (cudaStream_t)stream));
 }
 
+int mg_sigmakin_fused(mg_process* p, uint64_t seed, uint64_t first_event, int64_t n, void* d_me, void* d_ps_weight, void* d_event_weight, void* stream) {
+  if (!valid_handle(p) || n < 0) return MG_EINVAL;
+  if (n == 0) return MG_OK;
+  const size_t es = elem(p);
+  if (!d_me || !aligned(d_me, es) || (d_ps_weight && !aligned(d_ps_weight, es)) || (d_event_weight && !aligned(d_event_weight, es))) return MG_EINVAL;
+  DeviceGuard g(p->par.device); if (!g.ok) return MG_ECUDA;
+  cudaStream_t s = (cudaStream_t)stream;
+  if (p->par.process == MG_EEMUMU) return cuda_rc(launch_fused_eemumu(p, seed, first_event, n, d_me, d_ps_weight, d_event_weight, s));
+  if (p->par.process == MG_GGTT) return cuda_rc(launch_fused_ggtt(p, seed, first_event, n, d_me, d_ps_weight, d_event_weight, s));
+  // shared-memory recycling kernels: momenta go through the handle's scratch buffer (< 1 % of their time)
+  const int64_t ld = (n + 31) / 32 * 32;
+  const size_t mom_b = (size_t)4 * p->n_ext * ld * es, w_b = (size_t)ld * es;
+  int rc = ensure_scratch(p, mom_b + w_b, 0); if (rc != MG_OK) return rc;
+  char* d = (char*)p->d_scratch;
+  void* d_w = d_ps_weight ? d_ps_weight : (void*)(d + mom_b);
+  cudaError_t e = launch_generate(p, seed, first_event, n, ld, d, d_w, s);
+  if (e != cudaSuccess) return cuda_rc(e);
+  MeArgs a{d, n, ld, d_me, nullptr, nullptr, nullptr, p->hel_mask};
+  if (d_event_weight) { a.psw = d_w; a.evw = d_event_weight; }
+  return cuda_rc(launch_me(p, a, s));
+}
+
 int mg_sigmakin_per_helicity(mg_process* p, const void* d_momenta, int64_t n, int64_t ld, void* d_me_hel, void* stream) {
   int rc = check_soa(p, d_momenta, n, ld); if (rc != MG_OK || n == 0) return rc;
   rc = check_soa(p, d_me_hel, n, ld); if (rc != MG_OK) return rc;

@@ -55,6 +55,9 @@ cudaError_t launch_me_eemumu(const mg_process* p, const MeArgs& a, cudaStream_t 
 cudaError_t launch_me_ggtt(const mg_process* p, const MeArgs& a, cudaStream_t s);
 cudaError_t launch_me_ggttg(const mg_process* p, const MeArgs& a, cudaStream_t s);
 cudaError_t launch_me_ggttgg(const mg_process* p, const MeArgs& a, cudaStream_t s);
+// A1-A13 in one kernel (fused.cuh) for the one-thread-per-event processes
+cudaError_t launch_fused_eemumu(const mg_process* p, uint64_t seed, uint64_t first, int64_t n, void* me, void* psw, void* evw, cudaStream_t s);
+cudaError_t launch_fused_ggtt(const mg_process* p, uint64_t seed, uint64_t first, int64_t n, void* me, void* psw, void* evw, cudaStream_t s);
 // explicit flop tally of one helicity combination / fixed per-event overhead (generated)
 int64_t me_flops_per_helicity(int process);
 int64_t me_flops_per_event_fixed(int process);

@@ -301,3 +301,34 @@ def test_worked_examples_on_gpu(mg):
         mom[:, :1] = torch.tensor(aos_to_soa(ex["mom"]), device="cuda")
         me = P.sigmakin(mom, 1)[0].item()
         assert abs(me / ex["me"] - 1) < 1e-12
+
+
+# ----------------------------------------------------------------------------- A1-A13 fused
+@pytest.mark.parametrize("prec", [0, 1])
+@pytest.mark.parametrize("process", PROCS)
+def test_fused_path_matches_the_oracle_and_the_separate_kernels(mg, process, prec):
+    """mg_sigmakin_fused against (a) the oracle's own Philox -> RAMBO -> ME pipeline on the same (seed, event index)
+    and (b) mg_generate + mg_sigmakin of the library.  The fused kernels never store momenta, so (a) compares through
+    the whole chain: RAMBO rounding enters the ME, hence the looser per-event bound (C10) and the median check."""
+    n = {0: 8192 + 5, 1: 8192 + 5, 2: 2048 + 5, 3: 512 + 5}[process]
+    seed, first = 7, 1000
+    P = mg.Process(process, prec)
+    P.filter_helicities(P.generate(seed, first, 64)[0], 32)
+    w = torch.empty(n, dtype=P.dtype, device=P.device)
+    ew = torch.empty(n, dtype=P.dtype, device=P.device)
+    me = P.sigmakin_fused(seed, first, n, ps_weight=w, event_weight=ew)
+    mom, w2 = P.generate(seed, first, n)
+    me2 = P.sigmakin(mom, n)
+    tol = 1e-12 if prec == 0 else 2e-5
+    assert ((me / me2[:n]) - 1).abs().max().item() <= tol          # same device functions, two kernels
+    assert torch.equal(w, w2[:n]) or ((w / w2[:n]) - 1).abs().max().item() <= tol
+    assert ((ew / (w * me)) - 1).abs().max().item() <= (1e-15 if prec == 0 else 1e-6)
+    me_only = P.sigmakin_fused(seed, first, n)                     # optional outputs left out
+    assert torch.equal(me_only, me)
+    if prec == 0:                                                  # FP32 draws 23-bit uniforms (R3): other events
+        me_o, w_o = oracle.pipeline(process, seed, first, n)
+        rel = np.abs(me.cpu().numpy() / me_o - 1)
+        relw = np.abs(w.cpu().numpy() / w_o - 1)
+        print("fused process %d: ME max rel %.2e median %.2e, W max rel %.2e" % (process, rel.max(), np.median(rel), relw.max()))
+        assert np.median(rel) < 1e-13 and rel.max() < 1e-9 and relw.max() < 1e-9
+    assert P.sigmakin_fused(seed, first, 0) is not None            # n = 0 is a no-op
