@@ -222,6 +222,37 @@ def stage_rates(mg, torch, r, reps=20):
     return out
 
 
+def batch_sweep(mg, torch, name, device_index):
+    """Throughput against the number of events per launch (PAPER.md:104 Fig. 5 and its two definitions, :156-164:
+    kernel only, and kernel + device-to-host copy of the matrix elements)."""
+    process, prec, nmax, seed, cfg = WORKLOADS[name]
+    P = mg.Process(process, prec, device_index)
+    mom, w = P.generate(seed, 0, nmax)
+    P.filter_helicities(mom, 32)
+    me = torch.empty(mom.shape[1], dtype=P.dtype, device=P.device)
+    h_me = torch.empty(nmax, dtype=P.dtype).pin_memory()
+    n = 256
+    while n <= nmax:
+        reps = max(3, min(200, (1 << 22) // n))
+        for _ in range(3):
+            P.sigmakin(mom, n, me)
+        a, b, c = (torch.cuda.Event(enable_timing=True) for _ in range(3))
+        torch.cuda.synchronize()
+        a.record()
+        for _ in range(reps):
+            P.sigmakin(mom, n, me)
+        b.record()
+        for _ in range(reps):
+            P.sigmakin(mom, n, me)
+            h_me[:n].copy_(me[:n], non_blocking=True)
+        c.record()
+        torch.cuda.synchronize()
+        k_ms, kc_ms = a.elapsed_time(b) / reps, b.elapsed_time(c) / reps
+        print(json.dumps({"sweep": name, "events_per_launch": n, "kernel_ms": k_ms, "MEs_per_s_kernel": n / (k_ms * 1e-3),
+                          "MEs_per_s_kernel_plus_d2h": n / (kc_ms * 1e-3)}))
+        n *= 4
+
+
 def e2e_measure(mg, torch, r, steps):
     """End to end through the C ABI with HOST buffers: momenta H2D, sigmaKin, ME D2H (mg_sigmakin_host)."""
     P, n, ld = r["P"], r["n"], r["ld"]
@@ -247,7 +278,14 @@ def main():
     ap.add_argument("--workload", default="ggttgg_fp64", choices=sorted(WORKLOADS))
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-extra", action="store_true", help="skip the other workloads and the CPU baseline")
+    ap.add_argument("--sweep", action="store_true",
+                    help="batch-size sweep of the sigmaKin kernel (PAPER.md:104-108 Fig. 5): one JSON line per size, then exit")
     args = ap.parse_args()
+    if args.sweep:
+        import torch
+        import paper_2106_12631_b200 as mg
+        batch_sweep(mg, torch, args.workload, 0)
+        return
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.impl == "reference":
         run_reference(args)
