@@ -202,6 +202,18 @@ def stage_rates(mg, torch, r, reps=20):
     ew = torch.empty(ld, dtype=P.dtype, device=P.device)
     # A1-A13 in one call, momenta never stored: whole-path MEs/s next to the three-kernel step
     calls["fused_path"] = (lambda i: P.sigmakin_fused(r["seed"], i * n, n, me, w, ew), None)
+    # after the path: batch sums of the event weights and hit-or-miss stream compaction
+    fn_f = calls["fused_path"][0]
+    fn_f(0)
+    es = 8 if r["prec"] == 0 else 4
+    wmax = P.weight_sums(ew, n)[2]
+    kept = torch.empty(n, dtype=torch.int64, device=P.device)
+    nkept = [0]
+
+    def unw(i):
+        nkept[0] = len(P.unweight(r["seed"], 0, ew, n, wmax, kept))
+    calls["weight_sums"] = (lambda i: P.weight_sums(ew, n), n * es)
+    calls["unweight"] = (unw, None)
     out = {}
     for name, (fn, stage) in calls.items():
         for i in range(3):
@@ -214,8 +226,17 @@ def stage_rates(mg, torch, r, reps=20):
         b.record()
         torch.cuda.synchronize()
         ms = a.elapsed_time(b) / reps
-        if stage is None:
+        if name == "unweight":
+            stage = 2 * n * es + 8 * nkept[0]            # weights read by the count and the scatter pass, indices written
+            out_extra = {"kept": nkept[0], "of": n}
+        elif stage is None:
             out[name] = {"ms": ms, "MEs_per_s": n / (ms * 1e-3)}
+            continue
+        if name in ("weight_sums", "unweight"):          # synchronous calls: the time includes the host round trip
+            gbs = stage / (ms * 1e-3) / 1e9
+            out[name] = {"ms": ms, "GB/s": gbs, "frac_hbm": gbs / hbm if hbm else None, "events_per_s": n / (ms * 1e-3)}
+            if name == "unweight":
+                out[name].update(out_extra)
             continue
         gbs = n * P.bytes_per_event(stage) / (ms * 1e-3) / 1e9
         out[name] = {"ms": ms, "GB/s": gbs, "frac_hbm": gbs / hbm if hbm else None, "events_per_s": n / (ms * 1e-3)}

@@ -112,6 +112,24 @@ int mg_generate(mg_process* p, uint64_t seed, uint64_t first_event, int64_t n, i
 int mg_sigmakin_fused(mg_process* p, uint64_t seed, uint64_t first_event, int64_t n,
                       void* d_me, void* d_ps_weight, void* d_event_weight, void* stream);
 
+/* After the hot path ("a fiducial cross section ... and a sample of N_unw unweighted
+ * events", "event unweighting, where data stream compaction should in principle be straight-forward").
+ *
+ * mg_weight_sums: h_sums_out[0..2] = (sum w, sum w^2, max w) over the n non-negative event weights d_weights[n]
+ * (element type = the handle's precision), accumulated in double in a fixed order (bit-reproducible for a given n).
+ * The cross-section estimate of reading R27 is sum/n / (2 s) * 0.3893793721e9 pb, its MC error
+ * sqrt((sum2/n - (sum/n)^2)/n) times the same factor.  Synchronous on `stream` (returns host values).
+ *
+ * mg_unweight: hit-or-miss against w_max (R29): event e of the batch is kept iff u * w_max < w[e] in the weights'
+ * precision, u = word 0 of Philox4x32-10 with key = seed and counter (first_event + e, 0xFFFFFFFF, 0) mapped to (0,1)
+ * as in mg_rng (R28): the decision depends on the global event index only.  Writes the batch-relative indices of
+ * the kept events in increasing order to d_kept_out[0 .. *h_count_out) (caller allocates n int64) — a stable stream
+ * compaction, unique result.  Synchronous.  MG_EINVAL for w_max <= 0, NULL or misaligned pointers.
+ * Both use a device scratch buffer owned by the handle (grown on first use). */
+int mg_weight_sums(mg_process* p, const void* d_weights, int64_t n, double* h_sums_out, void* stream);
+int mg_unweight(mg_process* p, uint64_t seed, uint64_t first_event, const void* d_weights, int64_t n, double w_max,
+                int64_t* d_kept_out, int64_t* h_count_out, void* stream);
+
 /* A12: good-helicity filter (R16).  Evaluates every helicity combination on the
  * first probe_n events of d_momenta (1 <= probe_n <= n... the caller guarantees probe_n events are
  * present), marks h good iff max_e |M|^2_h / sum_h' |M|^2_h' > 1e-10, returns the mask in

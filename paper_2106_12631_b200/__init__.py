@@ -62,6 +62,8 @@ def lib():
         "mg_sigmakin": (C.c_int, [vp, vp, i64, i64, vp, vp, vp, vp]),
         "mg_sigmakin_per_helicity": (C.c_int, [vp, vp, i64, i64, vp, vp]),
         "mg_sigmakin_fused": (C.c_int, [vp, u64, u64, i64, vp, vp, vp, vp]),
+        "mg_weight_sums": (C.c_int, [vp, vp, i64, C.POINTER(C.c_double), vp]),
+        "mg_unweight": (C.c_int, [vp, u64, u64, vp, i64, C.c_double, vp, C.POINTER(i64), vp]),
         "mg_sigmakin_host": (C.c_int, [vp, vp, i64, i64, vp]),
         "mg_run_host": (C.c_int, [vp, u64, u64, i64, i64, vp, vp, vp]),
         "mg_flops_per_event": (i64, [vp, C.c_int]),
@@ -82,7 +84,7 @@ def lib():
 EXPORTED = ["mg_default_params", "mg_init_process", "mg_free_process", "mg_n_external", "mg_n_final", "mg_n_helicities",
             "mg_n_colour_flows", "mg_n_diagrams", "mg_n_amplitudes", "mg_me_denominator", "mg_colour_matrix",
             "mg_padded_stride", "mg_rng_words", "mg_rng", "mg_rambo", "mg_generate", "mg_filter_helicities",
-            "mg_set_helicity_mask", "mg_get_helicity_mask", "mg_sigmakin", "mg_sigmakin_per_helicity", "mg_sigmakin_fused",
+            "mg_set_helicity_mask", "mg_get_helicity_mask", "mg_sigmakin", "mg_sigmakin_per_helicity", "mg_sigmakin_fused", "mg_weight_sums", "mg_unweight",
             "mg_sigmakin_host", "mg_run_host", "mg_flops_per_event", "mg_bytes_per_event", "mg_last_kernel_ms",
             "mg_measure_alu_peak", "mg_measure_alu_mode", "mg_strerror", "mg_version"]
 
@@ -221,6 +223,19 @@ class Process:
                                        _ptr(ps_weight) if ps_weight is not None else None,
                                        _ptr(event_weight) if event_weight is not None else None, _stream(self.device)))
         return me
+
+    def weight_sums(self, weights, n):
+        """mg_weight_sums: (sum w, sum w^2, max w) of the first n event weights, in double."""
+        out = (C.c_double * 3)()
+        _check(lib().mg_weight_sums(self._h, _ptr(weights), n, out, _stream(self.device)))
+        return out[0], out[1], out[2]
+
+    def unweight(self, seed, first_event, weights, n, w_max, kept=None):
+        """mg_unweight: batch-relative indices of the events kept by hit-or-miss against w_max (int64 tensor view)."""
+        kept = kept if kept is not None else torch.empty(max(n, 1), dtype=torch.int64, device=self.device)
+        cnt = C.c_int64()
+        _check(lib().mg_unweight(self._h, seed, first_event, _ptr(weights), n, float(w_max), _ptr(kept), C.byref(cnt), _stream(self.device)))
+        return kept[:cnt.value]
 
     # ---- host-buffer (end-to-end) forms; tensors are CPU tensors (pinned for speed)
     def sigmakin_host(self, h_momenta, n, h_me):

@@ -13,7 +13,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libmg_b200.so")
-SOURCES = ["mg_api.cu", "rng_rambo.cu", "me_eemumu.cu", "me_ggtt.cu", "me_ggttg.cu", "me_ggttgg.cu", "me_tables.cu", "alu_peak.cu"]
+SOURCES = ["mg_api.cu", "rng_rambo.cu", "me_eemumu.cu", "me_ggtt.cu", "me_ggttg.cu", "me_ggttgg.cu", "me_tables.cu", "alu_peak.cu", "xsec.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "-Xptxas", "-v", "--fmad=true"] + os.environ.get("MG_NVCC_EXTRA", "").split()
 

@@ -226,6 +226,50 @@ int mg_sigmakin_fused(mg_process* p, uint64_t seed, uint64_t first_event, int64_
   return cuda_rc(launch_me(p, a, s));
 }
 
+int mg_weight_sums(mg_process* p, const void* d_weights, int64_t n, double* h_sums_out, void* stream) {
+  if (!valid_handle(p) || n < 0 || !h_sums_out) return MG_EINVAL;
+  h_sums_out[0] = h_sums_out[1] = h_sums_out[2] = 0.0;
+  if (n == 0) return MG_OK;
+  if (!d_weights || !aligned(d_weights, elem(p))) return MG_EINVAL;
+  DeviceGuard g(p->par.device); if (!g.ok) return MG_ECUDA;
+  cudaStream_t s = (cudaStream_t)stream;
+  const int64_t nb = weight_sums_blocks(n);
+  int rc = ensure_scratch(p, (size_t)nb * 3 * sizeof(double), 0); if (rc != MG_OK) return rc;
+  double* h = (double*)malloc((size_t)nb * 3 * sizeof(double));
+  if (!h) return MG_ENOMEM;
+  cudaError_t e = launch_weight_sums(p, d_weights, n, (double*)p->d_scratch, s);
+  if (e == cudaSuccess) e = cudaMemcpyAsync(h, p->d_scratch, (size_t)nb * 3 * sizeof(double), cudaMemcpyDeviceToHost, s);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(s);
+  if (e != cudaSuccess) { free(h); return cuda_rc(e); }
+  double s1 = 0, s2 = 0, mx = 0;
+  for (int64_t b = 0; b < nb; ++b) { s1 += h[3 * b]; s2 += h[3 * b + 1]; mx = h[3 * b + 2] > mx ? h[3 * b + 2] : mx; }   // block order: deterministic
+  free(h);
+  h_sums_out[0] = s1; h_sums_out[1] = s2; h_sums_out[2] = mx;
+  return MG_OK;
+}
+
+int mg_unweight(mg_process* p, uint64_t seed, uint64_t first_event, const void* d_weights, int64_t n, double w_max,
+                int64_t* d_kept_out, int64_t* h_count_out, void* stream) {
+  if (!valid_handle(p) || n < 0 || !h_count_out) return MG_EINVAL;
+  *h_count_out = 0;
+  if (n == 0) return MG_OK;
+  if (!d_weights || !aligned(d_weights, elem(p)) || !d_kept_out || !aligned(d_kept_out, sizeof(int64_t)) || !(w_max > 0.0)) return MG_EINVAL;
+  DeviceGuard g(p->par.device); if (!g.ok) return MG_ECUDA;
+  cudaStream_t s = (cudaStream_t)stream;
+  const int64_t nt = unweight_tiles(n);
+  const size_t off_b = (size_t)(nt + 1) * sizeof(int64_t), cnt_b = (size_t)nt * sizeof(int);
+  int rc = ensure_scratch(p, off_b + cnt_b, 0); if (rc != MG_OK) return rc;
+  int64_t* d_off = (int64_t*)p->d_scratch;
+  int* d_cnt = (int*)((char*)p->d_scratch + off_b);
+  cudaError_t e = launch_unweight(p, seed, first_event, d_weights, n, w_max, d_cnt, d_off, d_kept_out, s);
+  int64_t total = 0;
+  if (e == cudaSuccess) e = cudaMemcpyAsync(&total, d_off + nt, sizeof(int64_t), cudaMemcpyDeviceToHost, s);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(s);
+  if (e != cudaSuccess) return cuda_rc(e);
+  *h_count_out = total;
+  return MG_OK;
+}
+
 int mg_sigmakin_per_helicity(mg_process* p, const void* d_momenta, int64_t n, int64_t ld, void* d_me_hel, void* stream) {
   int rc = check_soa(p, d_momenta, n, ld); if (rc != MG_OK || n == 0) return rc;
   rc = check_soa(p, d_me_hel, n, ld); if (rc != MG_OK) return rc;

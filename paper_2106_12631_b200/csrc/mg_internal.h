@@ -58,6 +58,12 @@ cudaError_t launch_me_ggttgg(const mg_process* p, const MeArgs& a, cudaStream_t 
 // A1-A13 in one kernel (fused.cuh) for the one-thread-per-event processes
 cudaError_t launch_fused_eemumu(const mg_process* p, uint64_t seed, uint64_t first, int64_t n, void* me, void* psw, void* evw, cudaStream_t s);
 cudaError_t launch_fused_ggtt(const mg_process* p, uint64_t seed, uint64_t first, int64_t n, void* me, void* psw, void* evw, cudaStream_t s);
+// xsec.cu: batch sums of the event weights and hit-or-miss unweighting
+int64_t weight_sums_blocks(int64_t n);
+cudaError_t launch_weight_sums(const mg_process* p, const void* d_w, int64_t n, double* d_part, cudaStream_t s);
+int64_t unweight_tiles(int64_t n);
+cudaError_t launch_unweight(const mg_process* p, uint64_t seed, uint64_t first, const void* d_w, int64_t n, double wmax,
+                            int* d_counts, int64_t* d_offsets, int64_t* d_out, cudaStream_t s);
 // explicit flop tally of one helicity combination / fixed per-event overhead (generated)
 int64_t me_flops_per_helicity(int process);
 int64_t me_flops_per_event_fixed(int process);

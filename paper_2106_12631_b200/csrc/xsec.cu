@@ -1,0 +1,138 @@
+// xsec.cu — the two steps after the hot path: batch sums of the event weights
+// (cross-section estimate) and hit-or-miss unweighting with stream compaction.  Both are HBM-bound passes over
+// 8 (4) bytes per event; readings R27-R29 in DESIGN.md.
+//
+//   weight sums   one pass, every CTA reduces 1024 x ITEMS weights in double (fixed tree: thread-sequential, warp
+//                 butterfly, warps in order) and writes one partial (sum, sum of squares, max); the partials are
+//                 added on the host in block order -> deterministic for a given n.
+//   unweighting   pass 1 counts the kept events of every 1024-event tile, pass 2 is an exclusive scan of the tile
+//                 counts by one CTA, pass 3 recomputes the decisions (a Philox call is cheaper than storing flags)
+//                 and scatters the kept event indices in increasing order (ballot ranks inside a warp, warp
+//                 offsets inside the tile, tile offset from pass 2): a stable compaction, so the result is unique.
+#include "mg_internal.h"
+#include "philox.cuh"
+
+namespace mg {
+namespace {
+
+constexpr int kTile = 1024;
+constexpr int kItems = 8;          // weights per thread in the reduction
+
+template <class T>
+__global__ void __launch_bounds__(kTile) weight_sums_kernel(const T* __restrict__ w, int64_t n, double* __restrict__ part) {
+  __shared__ double sh[3][kTile / 32];
+  const int64_t base = (int64_t)blockIdx.x * kTile * kItems;
+  double s1 = 0, s2 = 0, mx = 0;
+#pragma unroll
+  for (int i = 0; i < kItems; ++i) {
+    const int64_t e = base + (int64_t)i * kTile + threadIdx.x;
+    if (e < n) {
+      const double x = (double)__ldcs(w + e);
+      s1 += x; s2 = fma(x, x, s2); mx = fmax(mx, x);
+    }
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+    s1 += __shfl_xor_sync(0xffffffffu, s1, o);
+    s2 += __shfl_xor_sync(0xffffffffu, s2, o);
+    mx = fmax(mx, __shfl_xor_sync(0xffffffffu, mx, o));
+  }
+  if ((threadIdx.x & 31) == 0) { sh[0][threadIdx.x >> 5] = s1; sh[1][threadIdx.x >> 5] = s2; sh[2][threadIdx.x >> 5] = mx; }
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    double a = 0, b = 0, c = 0;
+    for (int k = 0; k < kTile / 32; ++k) { a += sh[0][k]; b += sh[1][k]; c = fmax(c, sh[2][k]); }
+    part[3 * blockIdx.x + 0] = a; part[3 * blockIdx.x + 1] = b; part[3 * blockIdx.x + 2] = c;
+  }
+}
+
+// R28 + R29: is event e (global index first + e) kept?  u in (0,1) as in R3, decision in the weights' precision
+template <class T>
+__device__ __forceinline__ bool keep_event(uint64_t seed, uint64_t event, T w, T wmax) {
+  const u32x4 r = philox_event_particle(seed, event, 0xFFFFFFFFu);
+  return u32_to_uniform<T>(r.x) * wmax < w;
+}
+
+template <class T>
+__global__ void __launch_bounds__(kTile) unweight_count_kernel(uint64_t seed, uint64_t first, const T* __restrict__ w, int64_t n,
+                                                               T wmax, int* __restrict__ counts) {
+  const int64_t e = (int64_t)blockIdx.x * kTile + threadIdx.x;
+  const bool k = e < n && keep_event<T>(seed, first + (uint64_t)e, __ldg(w + e), wmax);
+  const int c = __syncthreads_count(k);
+  if (threadIdx.x == 0) counts[blockIdx.x] = c;
+}
+
+// exclusive scan of the tile counts by ONE CTA (at most 2^24 / 1024 = 16384 tiles per 2^24 events); total -> offsets[ntile]
+__global__ void __launch_bounds__(kTile) scan_counts_kernel(const int* __restrict__ counts, int64_t ntile, int64_t* __restrict__ offsets) {
+  __shared__ int64_t sh[kTile];
+  __shared__ int64_t carry;
+  if (threadIdx.x == 0) carry = 0;
+  __syncthreads();
+  for (int64_t b0 = 0; b0 < ntile; b0 += kTile) {
+    const int64_t i = b0 + threadIdx.x;
+    const int64_t v = i < ntile ? counts[i] : 0;
+    sh[threadIdx.x] = v;
+    __syncthreads();
+    for (int o = 1; o < kTile; o <<= 1) {                 // Hillis-Steele inclusive scan of one 1024-tile slab
+      const int64_t t = threadIdx.x >= o ? sh[threadIdx.x - o] : 0;
+      __syncthreads();
+      sh[threadIdx.x] += t;
+      __syncthreads();
+    }
+    if (i < ntile) offsets[i] = carry + sh[threadIdx.x] - v;
+    __syncthreads();
+    if (threadIdx.x == 0) carry += sh[kTile - 1];
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) offsets[ntile] = carry;
+}
+
+template <class T>
+__global__ void __launch_bounds__(kTile) unweight_scatter_kernel(uint64_t seed, uint64_t first, const T* __restrict__ w, int64_t n,
+                                                                 T wmax, const int64_t* __restrict__ offsets, int64_t* __restrict__ out) {
+  __shared__ int warp_base[kTile / 32];
+  const int64_t e = (int64_t)blockIdx.x * kTile + threadIdx.x;
+  const bool k = e < n && keep_event<T>(seed, first + (uint64_t)e, __ldg(w + e), wmax);
+  const unsigned b = __ballot_sync(0xffffffffu, k);
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+  if (lane == 0) warp_base[wid] = __popc(b);
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    int acc = 0;
+    for (int i = 0; i < kTile / 32; ++i) { const int c = warp_base[i]; warp_base[i] = acc; acc += c; }
+  }
+  __syncthreads();
+  if (k) out[offsets[blockIdx.x] + warp_base[wid] + __popc(b & ((1u << lane) - 1u))] = e;
+}
+
+}  // namespace
+
+// partials: 3 doubles per CTA in d_part (caller sizes it with weight_sums_blocks)
+int64_t weight_sums_blocks(int64_t n) { return (n + (int64_t)kTile * kItems - 1) / ((int64_t)kTile * kItems); }
+
+cudaError_t launch_weight_sums(const mg_process* p, const void* d_w, int64_t n, double* d_part, cudaStream_t s) {
+  const unsigned g = (unsigned)weight_sums_blocks(n);
+  if (p->par.precision == MG_FP64) weight_sums_kernel<double><<<g, kTile, 0, s>>>((const double*)d_w, n, d_part);
+  else weight_sums_kernel<float><<<g, kTile, 0, s>>>((const float*)d_w, n, d_part);
+  return cudaGetLastError();
+}
+
+int64_t unweight_tiles(int64_t n) { return (n + kTile - 1) / kTile; }
+
+// d_counts: int[ntile], d_offsets: int64[ntile + 1]; d_out: int64[n] (kept event indices, increasing)
+cudaError_t launch_unweight(const mg_process* p, uint64_t seed, uint64_t first, const void* d_w, int64_t n, double wmax,
+                            int* d_counts, int64_t* d_offsets, int64_t* d_out, cudaStream_t s) {
+  const int64_t nt = unweight_tiles(n);
+  if (p->par.precision == MG_FP64) {
+    unweight_count_kernel<double><<<(unsigned)nt, kTile, 0, s>>>(seed, first, (const double*)d_w, n, wmax, d_counts);
+    scan_counts_kernel<<<1, kTile, 0, s>>>(d_counts, nt, d_offsets);
+    unweight_scatter_kernel<double><<<(unsigned)nt, kTile, 0, s>>>(seed, first, (const double*)d_w, n, wmax, d_offsets, d_out);
+  } else {
+    unweight_count_kernel<float><<<(unsigned)nt, kTile, 0, s>>>(seed, first, (const float*)d_w, n, (float)wmax, d_counts);
+    scan_counts_kernel<<<1, kTile, 0, s>>>(d_counts, nt, d_offsets);
+    unweight_scatter_kernel<float><<<(unsigned)nt, kTile, 0, s>>>(seed, first, (const float*)d_w, n, (float)wmax, d_offsets, d_out);
+  }
+  return cudaGetLastError();
+}
+
+}  // namespace mg

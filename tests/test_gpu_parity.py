@@ -332,3 +332,51 @@ def test_fused_path_matches_the_oracle_and_the_separate_kernels(mg, process, pre
         print("fused process %d: ME max rel %.2e median %.2e, W max rel %.2e" % (process, rel.max(), np.median(rel), relw.max()))
         assert np.median(rel) < 1e-13 and rel.max() < 1e-9 and relw.max() < 1e-9
     assert P.sigmakin_fused(seed, first, 0) is not None            # n = 0 is a no-op
+
+
+# ----------------------------------------------------------------------------- after the path
+@pytest.mark.parametrize("prec", [0, 1])
+@pytest.mark.parametrize("n", [1, 1023, 1024, 8192 * 3 + 17])
+def test_weight_sums_and_unweighting_match_the_oracle(mg, prec, n):
+    """mg_weight_sums / mg_unweight against oracle/xsec.py: sums to 1e-12 (the oracle's are exactly rounded), the list
+    of kept events bit-exact (integer result; the decision u*w_max < w is taken in the weights' precision on both
+    sides, R29).  Sizes span one thread, a ragged tile, a full tile and several reduction blocks."""
+    from oracle import xsec
+    P = mg.Process(2, prec)
+    seed, first = 7, 2**33 + 11
+    ew = torch.empty(n, dtype=P.dtype, device=P.device)
+    P.sigmakin_fused(seed, first, n, event_weight=ew, ps_weight=torch.empty(n, dtype=P.dtype, device=P.device))
+    w = ew.cpu().numpy()
+    s1, s2, mx = P.weight_sums(ew, n)
+    o1, o2, omx = xsec.weight_sums(w)
+    assert abs(s1 / o1 - 1) < 1e-12 and abs(s2 / o2 - 1) < 1e-12 and mx == omx
+    for wmax in (mx, 0.37 * mx):                       # the batch maximum, and a cap that some weights exceed
+        kept = P.unweight(seed, first, ew, n, wmax).cpu().numpy()
+        ref = xsec.unweight(seed, first, w, wmax)
+        assert np.array_equal(kept, ref), (len(kept), len(ref))
+    assert len(P.unweight(seed, first, ew, 0, mx)) == 0
+    assert P.weight_sums(ew, 0) == (0.0, 0.0, 0.0)
+
+
+def test_unweighting_is_independent_of_the_batch_split_and_gives_the_cross_section(mg):
+    from oracle import xsec
+    P = mg.Process(1, 0)                                # g g -> t t~: closed-form total cross section (test_oracle_xsec.py)
+    n = 1 << 18
+    ew = torch.empty(n, dtype=P.dtype, device=P.device)
+    P.sigmakin_fused(7, 0, n, event_weight=ew, ps_weight=torch.empty(n, dtype=P.dtype, device=P.device))
+    s1, s2, mx = P.weight_sums(ew, n)
+    f = xsec.GEV2_TO_PB / (2 * SQRT_S**2)
+    sigma, err = f * s1 / n, f * np.sqrt(max(s2 / n - (s1 / n) ** 2, 0) / n)
+    par = oracle.default_params()
+    rho = 4 * par.mt**2 / SQRT_S**2
+    beta = np.sqrt(1 - rho)
+    ref = xsec.GEV2_TO_PB * np.pi * par.alpha_s**2 / (3 * SQRT_S**2) * (
+        (1 + rho + rho * rho / 16) * np.log((1 + beta) / (1 - beta)) - beta * (7 / 4 + 31 * rho / 16))
+    print("sigma(gg->tt~) = %.4f +- %.4f pb, closed form %.4f pb" % (sigma, err, ref))
+    assert abs(sigma - ref) < 4 * err
+    whole = P.unweight(7, 0, ew, n, mx)
+    h = n // 2 + 13
+    a = P.unweight(7, 0, ew[:h], h, mx)
+    b = P.unweight(7, h, ew[h:].clone(), n - h, mx) + h
+    assert torch.equal(torch.cat([a, b]), whole)
+    assert abs(len(whole) / n - s1 / n / mx) < 4 * np.sqrt(0.25 / n)     # acceptance = <w>/w_max
