@@ -380,3 +380,24 @@ def test_unweighting_is_independent_of_the_batch_split_and_gives_the_cross_secti
     b = P.unweight(7, h, ew[h:].clone(), n - h, mx) + h
     assert torch.equal(torch.cat([a, b]), whole)
     assert abs(len(whole) / n - s1 / n / mx) < 4 * np.sqrt(0.25 / n)     # acceptance = <w>/w_max
+
+
+# ----------------------------------------------------------------------------- FP32 robustness
+@pytest.mark.parametrize("process", PROCS)
+def test_fp32_error_profile(mg, process):
+    """single precision is attractive (>= 2x) but produced NaNs for about one event in a million and was
+    not validated.  This prints the error profile of the FP32 kernels (robust formulas of R19: propagator denominators
+    in double, P+pz without cancellation) against the FP64 oracle fed the same momenta, over a sample larger than the
+    parity test's, and asserts what north_star asks: no NaN, <= 1e-4 per event.  The table is kept in
+    profiles/r01_g_fp32_accuracy.md."""
+    n = {0: 1 << 18, 1: 1 << 17, 2: 1 << 14, 3: 1 << 12}[process]
+    P, mom, mom_aos, me_g, me_o = _me_compare(mg, process, 1, n, 7, first=10**6)
+    rel = np.abs(me_g / me_o - 1)
+    q = np.quantile(rel, [0.5, 0.99, 0.999])
+    print("fp32 profile process %d: n %d  median %.2e  p99 %.2e  p99.9 %.2e  max %.2e  mean bias %.2e  non-finite %d" % (
+        process, n, q[0], q[1], q[2], rel.max(), me_g.mean() / me_o.mean() - 1, (~np.isfinite(me_g)).sum()))
+    assert np.isfinite(me_g).all() and rel.max() <= 1e-4
+    # the large batch of config 2: 2^24 events through the fused FP32 path, no NaN / Inf / non-positive value
+    if process == 0:
+        me = P.sigmakin_fused(7, 0, 1 << 24)
+        assert bool(torch.isfinite(me).all().item()) and bool((me > 0).all().item())
