@@ -258,10 +258,11 @@ int mg_unweight(mg_process* p, uint64_t seed, uint64_t first_event, const void* 
   cudaStream_t s = (cudaStream_t)stream;
   const int64_t nt = unweight_tiles(n);
   const size_t off_b = (size_t)(nt + 1) * sizeof(int64_t), cnt_b = (size_t)nt * sizeof(int);
-  int rc = ensure_scratch(p, off_b + cnt_b, 0); if (rc != MG_OK) return rc;
+  int rc = ensure_scratch(p, off_b + cnt_b + (size_t)nt * 32 * sizeof(unsigned), 0); if (rc != MG_OK) return rc;
   int64_t* d_off = (int64_t*)p->d_scratch;
   int* d_cnt = (int*)((char*)p->d_scratch + off_b);
-  cudaError_t e = launch_unweight(p, seed, first_event, d_weights, n, w_max, d_cnt, d_off, d_kept_out, s);
+  unsigned* d_bal = (unsigned*)((char*)p->d_scratch + off_b + cnt_b);
+  cudaError_t e = launch_unweight(p, seed, first_event, d_weights, n, w_max, d_cnt, d_bal, d_off, d_kept_out, s);
   int64_t total = 0;
   if (e == cudaSuccess) e = cudaMemcpyAsync(&total, d_off + nt, sizeof(int64_t), cudaMemcpyDeviceToHost, s);
   if (e == cudaSuccess) e = cudaStreamSynchronize(s);

@@ -63,7 +63,7 @@ int64_t weight_sums_blocks(int64_t n);
 cudaError_t launch_weight_sums(const mg_process* p, const void* d_w, int64_t n, double* d_part, cudaStream_t s);
 int64_t unweight_tiles(int64_t n);
 cudaError_t launch_unweight(const mg_process* p, uint64_t seed, uint64_t first, const void* d_w, int64_t n, double wmax,
-                            int* d_counts, int64_t* d_offsets, int64_t* d_out, cudaStream_t s);
+                            int* d_counts, unsigned* d_ballots, int64_t* d_offsets, int64_t* d_out, cudaStream_t s);
 // explicit flop tally of one helicity combination / fixed per-event overhead (generated)
 int64_t me_flops_per_helicity(int process);
 int64_t me_flops_per_event_fixed(int process);

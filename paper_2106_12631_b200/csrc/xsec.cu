@@ -5,10 +5,11 @@
 //   weight sums   one pass, every CTA reduces 1024 x ITEMS weights in double (fixed tree: thread-sequential, warp
 //                 butterfly, warps in order) and writes one partial (sum, sum of squares, max); the partials are
 //                 added on the host in block order -> deterministic for a given n.
-//   unweighting   pass 1 counts the kept events of every 1024-event tile, pass 2 is an exclusive scan of the tile
-//                 counts by one CTA, pass 3 recomputes the decisions (a Philox call is cheaper than storing flags)
-//                 and scatters the kept event indices in increasing order (ballot ranks inside a warp, warp
-//                 offsets inside the tile, tile offset from pass 2): a stable compaction, so the result is unique.
+//   unweighting   pass 1 takes the decisions (one Philox call per event: this pass is bound by integer issue, not by
+//                 HBM), stores them as one ballot word per warp and counts the kept events of every 1024-event
+//                 tile; pass 2 is an exclusive scan of the tile counts by one CTA; pass 3 reads the ballots and
+//                 scatters the kept event indices in increasing order (ballot ranks inside a warp, warp offsets
+//                 inside the tile, tile offset from pass 2): a stable compaction, so the result is unique.
 #include "mg_internal.h"
 #include "philox.cuh"
 
@@ -55,46 +56,54 @@ __device__ __forceinline__ bool keep_event(uint64_t seed, uint64_t event, T w, T
 
 template <class T>
 __global__ void __launch_bounds__(kTile) unweight_count_kernel(uint64_t seed, uint64_t first, const T* __restrict__ w, int64_t n,
-                                                               T wmax, int* __restrict__ counts) {
+                                                               T wmax, int* __restrict__ counts, unsigned* __restrict__ ballots) {
   const int64_t e = (int64_t)blockIdx.x * kTile + threadIdx.x;
-  const bool k = e < n && keep_event<T>(seed, first + (uint64_t)e, __ldg(w + e), wmax);
+  const bool k = e < n && keep_event<T>(seed, first + (uint64_t)e, __ldcs(w + e), wmax);
+  const unsigned b = __ballot_sync(0xffffffffu, k);
+  if ((threadIdx.x & 31) == 0) ballots[e >> 5] = b;
   const int c = __syncthreads_count(k);
   if (threadIdx.x == 0) counts[blockIdx.x] = c;
 }
 
-// exclusive scan of the tile counts by ONE CTA (at most 2^24 / 1024 = 16384 tiles per 2^24 events); total -> offsets[ntile]
+// exclusive scan of the tile counts by ONE CTA (2^24 events = 16384 tiles): every thread owns a contiguous chunk,
+// the 1024 chunk sums are scanned with warp shuffles (two levels); total -> offsets[ntile]
 __global__ void __launch_bounds__(kTile) scan_counts_kernel(const int* __restrict__ counts, int64_t ntile, int64_t* __restrict__ offsets) {
-  __shared__ int64_t sh[kTile];
-  __shared__ int64_t carry;
-  if (threadIdx.x == 0) carry = 0;
-  __syncthreads();
-  for (int64_t b0 = 0; b0 < ntile; b0 += kTile) {
-    const int64_t i = b0 + threadIdx.x;
-    const int64_t v = i < ntile ? counts[i] : 0;
-    sh[threadIdx.x] = v;
-    __syncthreads();
-    for (int o = 1; o < kTile; o <<= 1) {                 // Hillis-Steele inclusive scan of one 1024-tile slab
-      const int64_t t = threadIdx.x >= o ? sh[threadIdx.x - o] : 0;
-      __syncthreads();
-      sh[threadIdx.x] += t;
-      __syncthreads();
-    }
-    if (i < ntile) offsets[i] = carry + sh[threadIdx.x] - v;
-    __syncthreads();
-    if (threadIdx.x == 0) carry += sh[kTile - 1];
-    __syncthreads();
+  __shared__ int64_t warp_sum[kTile / 32];
+  const int64_t chunk = (ntile + kTile - 1) / kTile;
+  const int64_t lo = (int64_t)threadIdx.x * chunk, hi = lo + chunk < ntile ? lo + chunk : ntile;
+  int64_t mine = 0;
+  for (int64_t i = lo; i < hi; ++i) mine += counts[i];
+  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+  int64_t incl = mine;                                    // inclusive scan inside the warp
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) {
+    const int64_t t = __shfl_up_sync(0xffffffffu, incl, o);
+    if (lane >= o) incl += t;
   }
-  if (threadIdx.x == 0) offsets[ntile] = carry;
+  if (lane == 31) warp_sum[wid] = incl;
+  __syncthreads();
+  if (wid == 0) {
+    int64_t v = warp_sum[lane], sc = v;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      const int64_t t = __shfl_up_sync(0xffffffffu, sc, o);
+      if (lane >= o) sc += t;
+    }
+    warp_sum[lane] = sc - v;                              // exclusive prefix of the warps
+  }
+  __syncthreads();
+  int64_t run = warp_sum[wid] + incl - mine;              // exclusive prefix of this thread's chunk
+  for (int64_t i = lo; i < hi; ++i) { offsets[i] = run; run += counts[i]; }
+  if (threadIdx.x == kTile - 1) offsets[ntile] = warp_sum[wid] + incl;
 }
 
-template <class T>
-__global__ void __launch_bounds__(kTile) unweight_scatter_kernel(uint64_t seed, uint64_t first, const T* __restrict__ w, int64_t n,
-                                                                 T wmax, const int64_t* __restrict__ offsets, int64_t* __restrict__ out) {
+__global__ void __launch_bounds__(kTile) unweight_scatter_kernel(const unsigned* __restrict__ ballots, const int64_t* __restrict__ offsets,
+                                                                 int64_t* __restrict__ out) {
   __shared__ int warp_base[kTile / 32];
   const int64_t e = (int64_t)blockIdx.x * kTile + threadIdx.x;
-  const bool k = e < n && keep_event<T>(seed, first + (uint64_t)e, __ldg(w + e), wmax);
-  const unsigned b = __ballot_sync(0xffffffffu, k);
   const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+  const unsigned b = __ldg(ballots + (e >> 5));          // one word per warp (events beyond n have a zero bit)
+  const bool k = (b >> lane) & 1u;
   if (lane == 0) warp_base[wid] = __popc(b);
   __syncthreads();
   if (threadIdx.x == 0) {
@@ -119,19 +128,17 @@ cudaError_t launch_weight_sums(const mg_process* p, const void* d_w, int64_t n, 
 
 int64_t unweight_tiles(int64_t n) { return (n + kTile - 1) / kTile; }
 
-// d_counts: int[ntile], d_offsets: int64[ntile + 1]; d_out: int64[n] (kept event indices, increasing)
+// d_counts: int[ntile], d_ballots: unsigned[32 * ntile], d_offsets: int64[ntile + 1]; d_out: int64[n] (kept event indices, increasing)
 cudaError_t launch_unweight(const mg_process* p, uint64_t seed, uint64_t first, const void* d_w, int64_t n, double wmax,
-                            int* d_counts, int64_t* d_offsets, int64_t* d_out, cudaStream_t s) {
+                            int* d_counts, unsigned* d_ballots, int64_t* d_offsets, int64_t* d_out, cudaStream_t s) {
   const int64_t nt = unweight_tiles(n);
   if (p->par.precision == MG_FP64) {
-    unweight_count_kernel<double><<<(unsigned)nt, kTile, 0, s>>>(seed, first, (const double*)d_w, n, wmax, d_counts);
-    scan_counts_kernel<<<1, kTile, 0, s>>>(d_counts, nt, d_offsets);
-    unweight_scatter_kernel<double><<<(unsigned)nt, kTile, 0, s>>>(seed, first, (const double*)d_w, n, wmax, d_offsets, d_out);
+    unweight_count_kernel<double><<<(unsigned)nt, kTile, 0, s>>>(seed, first, (const double*)d_w, n, wmax, d_counts, d_ballots);
   } else {
-    unweight_count_kernel<float><<<(unsigned)nt, kTile, 0, s>>>(seed, first, (const float*)d_w, n, (float)wmax, d_counts);
-    scan_counts_kernel<<<1, kTile, 0, s>>>(d_counts, nt, d_offsets);
-    unweight_scatter_kernel<float><<<(unsigned)nt, kTile, 0, s>>>(seed, first, (const float*)d_w, n, (float)wmax, d_offsets, d_out);
+    unweight_count_kernel<float><<<(unsigned)nt, kTile, 0, s>>>(seed, first, (const float*)d_w, n, (float)wmax, d_counts, d_ballots);
   }
+  scan_counts_kernel<<<1, kTile, 0, s>>>(d_counts, nt, d_offsets);
+  unweight_scatter_kernel<<<(unsigned)nt, kTile, 0, s>>>(d_ballots, d_offsets, d_out);
   return cudaGetLastError();
 }
 
