@@ -374,7 +374,7 @@ def main():
             out["stages"] = stage_rates(mg, torch, r)
         except Exception as e:
             out["stages"] = "failed: %s" % e
-        tr = os.path.join(ROOT, "profiles", "traffic.json")
+        tr = os.path.join(ROOT, "profiles", "traffic.json.txt")
         if os.path.exists(tr):
             out["roofline"]["traffic"] = json.load(open(tr)).get(args.workload)
     if rank == 0 and world == 1 and not args.no_extra:
