@@ -46,7 +46,7 @@ struct TermDesc {   // one term of a gluon current: type 0: V3(A,kA,B,kB);  1..3
   unsigned int signbit;   // 0 or 0x80000000: the term enters with sign -1
   Op op[3];
 };
-struct MomDef { signed char c[6]; signed char propkind; signed char pad; };   // momentum = sum_i c[i] p_i ; 0 none, 1: 1/q^2, 2: 1/(q^2-mt^2)
+struct __align__(8) MomDef { signed char c[6]; signed char propkind; signed char pad; };   // momentum = sum_i c[i] p_i ; 0 none, 1: 1/q^2, 2: 1/(q^2-mt^2)
 
 template <class T> struct V2;
 template <> struct V2<double> { typedef double2 type; };
@@ -222,18 +222,23 @@ template <class P, class T> __device__ __forceinline__ void run_momtab(const Sme
   if (t >= P::E * P::NMOM) return;
   const int e = t / P::NMOM, m = t - e * P::NMOM;
   const MomDef d = P::momdef(m);
+  // the six coefficients (+1 / -1 / 0) arrive as ONE 8-byte constant load and become doubles by bit assembly: no
+  // per-coefficient constant load and integer-to-double conversion on the critical path of the first phase
+  const unsigned long long dw = *reinterpret_cast<const unsigned long long*>(&d);
   double q[4] = {0, 0, 0, 0};
 #pragma unroll
   for (int j = 0; j < P::NPAR; ++j) {
-    const double c = (double)d.c[j];
+    const int cj = (int)(signed char)((dw >> (8 * j)) & 0xffull);
+    const double c = __hiloint2double(cj == 0 ? 0 : (cj > 0 ? 0x3ff00000 : (int)0xbff00000), 0);
 #pragma unroll
     for (int mu = 0; mu < 4; ++mu) q[mu] = fma(c, (double)s.ext[(e * P::NPAR + j) * 4 + mu], q[mu]);
   }
 #pragma unroll
   for (int mu = 0; mu < 4; ++mu) s.mom[(e * P::NMOM + m) * 4 + mu] = (T)q[mu];
   double den = fma(q[0], q[0], fma(-q[1], q[1], fma(-q[2], q[2], -q[3] * q[3])));
-  if (d.propkind == 2) den = fma(-(double)mt, (double)mt, den);
-  s.ip[e * P::NMOM + m] = d.propkind ? (T)(1.0 / den) : (T)0;
+  const int propkind = (int)((dw >> 48) & 0xffull);
+  if (propkind == 2) den = fma(-(double)mt, (double)mt, den);
+  s.ip[e * P::NMOM + m] = propkind ? (T)(1.0 / den) : (T)0;
 }
 
 // ---------------------------------------------------------------------------------------------------
