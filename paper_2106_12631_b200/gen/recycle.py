@@ -104,7 +104,7 @@ class Program:
         self._build_momenta()
         self._build_nodes()
         self._build_closures()
-        self._schedule(chunk_budget)
+        self._schedule(int(os.environ.get('MG_RC%d_BUDGET' % ng, chunk_budget)))
         self._allocate()
         self._tally()
 
