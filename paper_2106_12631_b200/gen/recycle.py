@@ -88,7 +88,7 @@ class Closure:
 
 
 class Program:
-    def __init__(self, ng, chunk_budget=200):
+    def __init__(self, ng, chunk_budget=240):
         self.ng = ng
         g = self.g = qcdgen.Generator(ng)
         self.npar = ng + 2
@@ -232,7 +232,11 @@ class Program:
             nn = new_node(c)
             classes.setdefault((nn.nbits, nn.kind), OrderedDict()).setdefault(nn.name, []).append(c)
         chunks, cur, cur_n = [], [], 0
-        for key in sorted(classes):
+        keys = sorted(classes)
+        perm = os.environ.get('MG_RC%d_ORDER' % self.ng)          # sweep knob: order of the closure classes
+        if perm:
+            keys = [keys[int(ch)] for ch in perm]
+        for key in keys:
             names = list(classes[key])
             total = sum(self.half[x].nvar for x in names)
             if total > budget:                              # split a large class into equal parts
