@@ -99,12 +99,26 @@ class Program:
         self.E = int(os.environ.get('MG_RC%d_E' % ng, dflt[0]))
         self.MINB = int(os.environ.get('MG_RC%d_MINB' % ng, dflt[1]))
         self.MINB32 = int(os.environ.get('MG_RC%d_MINB32' % ng, dflt[2]))
+        # closure steps (indices into self.steps) that are NOT followed by a barrier: 'auto' = every one whose inputs can
+        # be held through the next producer step without more shared memory; 'all', '0' (none) or a list for sweeps
+        self.RELAXED = os.environ.get('MG_RC%d_RELAXED' % ng, 'auto')
         self.NT = self.E * self.nhel
         self.gp = g.gl_particle
         self._build_momenta()
         self._build_nodes()
         self._build_closures()
         self._schedule(int(os.environ.get('MG_RC%d_BUDGET' % ng, chunk_budget)))
+        if self.RELAXED == 'auto':
+            self.RELAXED = '0'
+            self._allocate()
+            base, chosen = self.nslot, []
+            for si, (kind, _) in enumerate(self.steps[:-1]):
+                if kind == "F":
+                    self.RELAXED = ",".join(map(str, chosen + [si]))
+                    self._allocate()
+                    if self.nslot <= base:
+                        chosen.append(si)
+            self.RELAXED = ",".join(map(str, chosen)) or '0'
         self._allocate()
         self._tally()
 
@@ -305,10 +319,19 @@ class Program:
             for o in n.operands():
                 assert o.born < n.born
 
+    def relaxed(self, si):
+        if self.steps[si][0] != "F" or not self.RELAXED or self.RELAXED == '0':
+            return False
+        return self.RELAXED in ('all', '1') or str(si) in self.RELAXED.split(',')
+
     # ------------------------------------------------------------------ shared-memory entries by liveness
     def _allocate(self):
         live = []          # (slot, size, last)
         self.nslot = 0
+        # RELAXED: no barrier between a closure step and the producer step after it, so that producer step must not
+        # overwrite what the closure step reads: such entries are held one step longer
+        def hold(n):
+            return n.last + 1 if self.relaxed(n.last) else n.last
         for n in self.all_nodes:
             live = [iv for iv in live if iv[2] >= n.born]          # entries whose last reader ran in an earlier step are free
             align = min(n.nvar, 8)
@@ -318,7 +341,7 @@ class Program:
                     break
                 pos = max(pos, (s + size + align - 1) // align * align)
             n.slot = pos
-            live.append((pos, n.nvar, n.last))
+            live.append((pos, n.nvar, hold(n)))
             self.nslot = max(self.nslot, pos + n.nvar)
         self.nslot = (self.nslot + 7) // 8 * 8
 
@@ -479,7 +502,7 @@ def emit(prog):
                 w("        }")
             w("      }")
             w("    }")
-            if si != len(prog.steps) - 1:
+            if si != len(prog.steps) - 1 and not prog.relaxed(si):
                 w("    __syncthreads();")
     assert len(seen) == nf
     num, den = prog.num, prog.den
