@@ -209,18 +209,25 @@ template <class P, class T> struct Smem {
 };
 
 // task t of a group of `nfam` nodes that all have NB helicity bits: t -> (node, event, variant), variant fastest
-template <class P, class T, int KIND, int NB> __device__ __forceinline__ void run_group(const Smem<P, T>& s, int first_node, int nfam, int t, T mt) {
-  constexpr int PER = P::E << NB;
+// A CTA holds E events in E / EG GROUPS of EG events; a group's threads share its tasks and its barrier, groups never
+// exchange data (ebase = first event of the thread's group).
+template <class P, class T, int KIND, int NB> __device__ __forceinline__ void run_group(const Smem<P, T>& s, int first_node, int nfam, int t, T mt, int ebase) {
+  constexpr int PER = P::EG << NB;
   const int fam = t / PER;
   if (fam >= nfam) return;
   const int r = t - fam * PER, v = r & ((1 << NB) - 1);
-  Task<P, T, KIND>::run(P::node(first_node + fam), v, s.pext4[v], s.view(r >> NB), mt);
+  Task<P, T, KIND>::run(P::node(first_node + fam), v, s.pext4[v], s.view(ebase + (r >> NB)), mt);
+}
+// barrier over the threads of one group
+template <class P> __device__ __forceinline__ void sync_group(int grp) {
+  if (P::EG == P::E || (P::EG * P::NHEL) % 32 != 0) __syncthreads();
+  else asm volatile("bar.sync %0, %1;" ::"r"(grp + 1), "n"(P::EG * P::NHEL) : "memory");
 }
 // line momenta (signed sums of external momenta) and inverse propagator denominators, in double also for
 // T = float (once per event; k_i.k_j cancels like theta^2 for collinear pairs, R19).  Task t = (event, entry).
-template <class P, class T> __device__ __forceinline__ void run_momtab(const Smem<P, T>& s, int t, T mt) {
-  if (t >= P::E * P::NMOM) return;
-  const int e = t / P::NMOM, m = t - e * P::NMOM;
+template <class P, class T> __device__ __forceinline__ void run_momtab(const Smem<P, T>& s, int t, T mt, int ebase) {
+  if (t >= P::EG * P::NMOM) return;
+  const int e = ebase + t / P::NMOM, m = t - (t / P::NMOM) * P::NMOM;
   const MomDef d = P::momdef(m);
   // the six coefficients (+1 / -1 / 0) arrive as ONE 8-byte constant load and become doubles by bit assembly: no
   // per-coefficient constant load and integer-to-double conversion on the critical path of the first phase
@@ -284,7 +291,7 @@ __global__ void __launch_bounds__(P::NT, sizeof(T) == 8 ? P::MINB : P::MINB32) s
   for (int o = LANES / 2; o > 0; o >>= 1) me_h += __shfl_xor_sync(0xffffffffu, me_h, o);
   if (P::NHEL > 32) {
     if ((tid & 31) == 0) s.red[tid >> 5] = me_h;
-    __syncthreads();
+    sync_group<P>(tid / (P::EG * P::NHEL));
     if (h == 0) {
       me_h = (T)0;
 #pragma unroll

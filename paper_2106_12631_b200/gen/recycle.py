@@ -99,9 +99,15 @@ class Program:
         self.E = int(os.environ.get('MG_RC%d_E' % ng, dflt[0]))
         self.MINB = int(os.environ.get('MG_RC%d_MINB' % ng, dflt[1]))
         self.MINB32 = int(os.environ.get('MG_RC%d_MINB32' % ng, dflt[2]))
+        # events per synchronisation group inside a CTA (divides E): the groups of a CTA share nothing but its code
+        self.EG = int(os.environ.get('MG_RC%d_EG' % ng, self.E))
+        assert self.E % self.EG == 0
         # closure steps (indices into self.steps) that are NOT followed by a barrier: 'auto' = every one whose inputs can
         # be held through the next producer step without more shared memory; 'all', '0' (none) or a list for sweeps
         self.RELAXED = os.environ.get('MG_RC%d_RELAXED' % ng, 'auto')
+        # shared-memory entries per event that still let E events x MINB CTAs share an SM (hoisting and barrier removal
+        # may spend them); 0: never more than the schedule needs anyway
+        self.SLOT_LIMIT = int(os.environ.get('MG_RC%d_SLOTS' % ng, {4: 424}.get(ng, 0)))
         self.NT = self.E * self.nhel
         self.gp = g.gl_particle
         self._build_momenta()
@@ -116,7 +122,7 @@ class Program:
                 if kind == "F":
                     self.RELAXED = ",".join(map(str, chosen + [si]))
                     self._allocate()
-                    if self.nslot <= base:
+                    if self.nslot <= max(base, self.SLOT_LIMIT):
                         chosen.append(si)
             self.RELAXED = ",".join(map(str, chosen)) or '0'
         self._allocate()
@@ -300,7 +306,49 @@ class Program:
                     self.steps.append(("P", list(ps)))
             # closures sharing the second operand are adjacent: it is loaded once
             self.steps.append(("F", sorted(ch, key=lambda c: (c.b.name, c.a.name))))
+        self._number()
+        # HOIST: a producer step whose nodes can all be computed in an earlier producer step (operands born before it)
+        # rides with that step when this costs no shared memory: one barrier-separated latency chain fewer
+        if os.environ.get('MG_RC%d_HOIST' % self.ng, '1') != '0':
+            self.RELAXED_SAVE, self.RELAXED = self.RELAXED, '0'
+            self._allocate()
+            limit = max(self.nslot, self.SLOT_LIMIT)
+            si = 1
+            while si < len(self.steps):
+                kind, items = self.steps[si]
+                moved = False
+                if kind == "P":
+                    ready = max(o.born for n in items for o in n.operands()) if any(n.operands() for n in items) else -1
+                    cands = [sj for sj in range(si - 1, ready, -1) if self.steps[sj][0] == "P"]
+                    for sj in cands:
+                        trial = [(k, list(it)) for k, it in self.steps]
+                        trial[sj][1].extend(items)
+                        del trial[si]
+                        # two closure steps that become adjacent merge into one
+                        merged = []
+                        for k, it in trial:
+                            if merged and k == "F" and merged[-1][0] == "F":
+                                merged[-1] = ("F", sorted(merged[-1][1] + it, key=lambda c: (c.b.name, c.a.name)))
+                            else:
+                                merged.append((k, it))
+                        keep = self.steps
+                        self.steps = merged
+                        self._number()
+                        self._allocate()
+                        if self.nslot <= limit:
+                            moved = True
+                            break
+                        self.steps = keep
+                        self._number()
+                if not moved:
+                    si += 1
+            self.RELAXED = self.RELAXED_SAVE
+            self._number()
+
+    def _number(self):
         # birth / last use
+        for n in list(self.nodes.values()) + list(self.half.values()):
+            n.born = n.last = None
         for si, (kind, items) in enumerate(self.steps):
             if kind == "P":
                 for n in items:
@@ -445,7 +493,7 @@ def emit(prog):
         w(l)
     w("};")
     w("struct %s {" % name)
-    w("  static constexpr int NPAR = %d, NHEL = %d, NFLOW = %d, E = %d, NT = %d, MINB = %d, MINB32 = %d;" % (npar, prog.nhel, nf, prog.E, prog.NT, prog.MINB, prog.MINB32))
+    w("  static constexpr int NPAR = %d, NHEL = %d, NFLOW = %d, E = %d, EG = %d, NT = %d, NTG = %d, MINB = %d, MINB32 = %d;" % (npar, prog.nhel, nf, prog.E, prog.EG, prog.NT, prog.EG * prog.nhel, prog.MINB, prog.MINB32))
     w("  static constexpr int NMOM = %d, NSLOT = %d;" % (len(prog.mom_defs), prog.nslot))
     w("  static __device__ __forceinline__ const rc::NodeDesc& node(int i) { return kRcNode_%s[i]; }" % tag)
     w("  static __device__ __forceinline__ const rc::TermDesc& term(int i) { return kRcTerm_%s[i]; }" % tag)
@@ -454,6 +502,7 @@ def emit(prog):
     w("  // producer steps, inner products, colour sum: |M|^2 of helicity h of event el (no g_s^(2 n_g)/denominator)")
     w("  template <class T> static __device__ __forceinline__ T run(const rc::Smem<%s, T>& s, int tid, int el, int h, T mt) {" % name)
     w("    const rc::View<T, NSLOT> ev = s.view(el);")
+    w("    const int grp = tid / NTG, gt = tid - grp * NTG, eb = grp * EG;   // synchronisation group, thread in it, its first event")
     w("    cx<T> jamp[NFLOW];")
     seen = set()
     for si, (kind, items) in enumerate(prog.steps):
@@ -461,24 +510,24 @@ def emit(prog):
             gr = Program.groups(items)
             bounds, b = [], 0
             if si == 0:                                   # line momenta and propagators ride with the external wavefunctions
-                cnt = prog.E * len(prog.mom_defs)
+                cnt = prog.EG * len(prog.mom_defs)
                 bounds.append(("MOMTAB", 0, 0, 0, 0, (cnt + 31) // 32 * 32))
                 b = bounds[0][5]
             for (k, nb), ns in gr.items():
-                cnt = len(ns) * (prog.E << nb)
+                cnt = len(ns) * (prog.EG << nb)
                 pad = (cnt + 31) // 32 * 32
                 bounds.append((k, nb, index[ns[0].name], len(ns), b, b + pad))
                 b += pad
             w("    // step %d: %s%s" % (si, "momentum table, " if si == 0 else "", ", ".join("%d x %s/%d bits" % (len(ns), k, nb) for (k, nb), ns in gr.items())))
-            w("    for (int t = tid; t < %d; t += NT) {" % b)
+            w("    for (int t = gt; t < %d; t += NTG) {" % b)
             for i, (k, nb, first, nfam, lo, hi) in enumerate(bounds):
                 cond = "" if len(bounds) == 1 else ("if (t < %d) " % hi if i == 0 else ("else if (t < %d) " % hi if i < len(bounds) - 1 else "else "))
                 if k == "MOMTAB":
-                    w("      %src::run_momtab<%s, T>(s, t, mt);" % (cond, name))
+                    w("      %src::run_momtab<%s, T>(s, t, mt, eb);" % (cond, name))
                 else:
-                    w("      %src::run_group<%s, T, rc::K_%s, %d>(s, %d, %d, t - %d, mt);" % (cond, name, k, nb, first, nfam, lo))
+                    w("      %src::run_group<%s, T, rc::K_%s, %d>(s, %d, %d, t - %d, mt, eb);" % (cond, name, k, nb, first, nfam, lo))
             w("    }")
-            w("    __syncthreads();")
+            w("    rc::sync_group<%s>(grp);" % name)
         else:
             w("    // step %d: %d inner products" % (si, len(items)))
             cur_b = None
@@ -503,7 +552,7 @@ def emit(prog):
             w("      }")
             w("    }")
             if si != len(prog.steps) - 1 and not prog.relaxed(si):
-                w("    __syncthreads();")
+                w("    rc::sync_group<%s>(grp);" % name)
     assert len(seen) == nf
     num, den = prog.num, prog.den
     w("    // A10: colour sum  sum_f C_ff |J_f|^2 + 2 sum_{f<g} C_fg Re(J_f^* J_g),  C = numerators / %d" % den)
