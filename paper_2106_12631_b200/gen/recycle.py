@@ -525,7 +525,10 @@ def emit(prog):
                 if k == "MOMTAB":
                     w("      %src::run_momtab<%s, T>(s, t, mt, eb);" % (cond, name))
                 else:
-                    w("      %src::run_group<%s, T, rc::K_%s, %d>(s, %d, %d, t - %d, mt, eb);" % (cond, name, k, nb, first, nfam, lo))
+                    if k in os.environ.get("MG_RC_ABLATE", "").split(","):
+                        w("      %s{ }" % cond)
+                    else:
+                        w("      %src::run_group<%s, T, rc::K_%s, %d>(s, %d, %d, t - %d, mt, eb);" % (cond, name, k, nb, first, nfam, lo))
             w("    }")
             w("    rc::sync_group<%s>(grp);" % name)
         else:
