@@ -77,7 +77,8 @@ template <int MASK> __device__ __forceinline__ int pextc(int v) {
 // view of one event's shared memory
 template <class T, int NSLOT> struct View {
   typedef typename V2<T>::type W;
-  const T* ext;    // [NPAR][4]  external momenta as loaded
+  const T* gm;     // the event's column of the caller's momenta array (row stride gld): externals are read once, by step 0
+  int64_t gld;
   const T* mom;    // [NMOM][4]  line momenta
   const T* ip;     // [NMOM]     inverse propagator denominators
   W* ent;          // [4][NSLOT]
@@ -88,7 +89,12 @@ template <class T, int NSLOT> struct View {
   __device__ __forceinline__ void stv(int i, const Vec4<T>& v) const { st(0, i, v.v[0]); st(1, i, v.v[1]); st(2, i, v.v[2]); st(3, i, v.v[3]); }
   __device__ __forceinline__ void sts(int i, const Spinor<T>& s) const { st(0, i, s.l[0]); st(1, i, s.l[1]); st(2, i, s.r[0]); st(3, i, s.r[1]); }
   __device__ __forceinline__ Mom<T> ldm(int m) const { return ld4(mom + 4 * m); }
-  __device__ __forceinline__ Mom<T> ldx(int i) const { return ld4(ext + 4 * i); }
+  __device__ __forceinline__ Mom<T> ldx(int i) const {
+    Mom<T> p;
+#pragma unroll
+    for (int mu = 0; mu < 4; ++mu) p.v[mu] = __ldg(gm + (int64_t)(4 * i + mu) * gld);
+    return p;
+  }
   static __device__ __forceinline__ Mom<T> ld4(const T* q) {
     const W a = reinterpret_cast<const W*>(q)[0], b = reinterpret_cast<const W*>(q)[1];
     Mom<T> p; p.v[0] = a.x; p.v[1] = a.y; p.v[2] = b.x; p.v[3] = b.y; return p;
@@ -185,25 +191,27 @@ MG_RC_TASK(K_SLASHROW) {  // half product psibar Vslash (op0 = psibar, op1 = V)
 template <class P, class T> struct Smem {
   typedef typename V2<T>::type W;
   unsigned long long* pext4;   // [16]  nibble m of word v = pext(v, m)
-  T* ext;   // [E][NPAR*4]   external momenta as loaded
+  const T* gmom;   // caller's momenta, column of the CTA's first event; ld, nev: row stride, events of this CTA that exist
+  int64_t ld;
+  int nev;
   T* mom;   // [E][NMOM][4]
   T* ip;    // [E][NMOM]
   W* ent;   // [E][4][NSLOT]
   T* red;   // [NT/32]
-  static constexpr size_t kScalars = (size_t)P::E * (P::NPAR * 4 + P::NMOM * 5);
+  static constexpr size_t kScalars = (size_t)P::E * (P::NMOM * 5);
   static constexpr size_t kEntOff = 128 + (kScalars * sizeof(T) + 15) / 16 * 16;
   static constexpr size_t bytes() { return kEntOff + (size_t)P::E * 4 * P::NSLOT * sizeof(W) + (P::NT / 32) * sizeof(T) + 16; }
   __device__ __forceinline__ void bind(unsigned char* raw) {
     pext4 = reinterpret_cast<unsigned long long*>(raw);
-    ext = reinterpret_cast<T*>(raw + 128);
-    mom = ext + P::E * P::NPAR * 4;
+    mom = reinterpret_cast<T*>(raw + 128);
     ip = mom + P::E * P::NMOM * 4;
     ent = reinterpret_cast<W*>(raw + kEntOff);
     red = reinterpret_cast<T*>(ent + P::E * 4 * P::NSLOT);
   }
   __device__ __forceinline__ View<T, P::NSLOT> view(int e) const {
     View<T, P::NSLOT> v;
-    v.ext = ext + e * P::NPAR * 4; v.mom = mom + e * P::NMOM * 4; v.ip = ip + e * P::NMOM; v.ent = ent + e * 4 * P::NSLOT;
+    v.gm = gmom + (e < nev ? e : nev - 1); v.gld = ld;     // tail events re-read the last event and are not stored
+    v.mom = mom + e * P::NMOM * 4; v.ip = ip + e * P::NMOM; v.ent = ent + e * 4 * P::NSLOT;
     return v;
   }
 };
@@ -229,6 +237,7 @@ template <class P, class T> __device__ __forceinline__ void run_momtab(const Sme
   if (t >= P::EG * P::NMOM) return;
   const int e = ebase + t / P::NMOM, m = t - (t / P::NMOM) * P::NMOM;
   const MomDef d = P::momdef(m);
+  const T* gm = s.gmom + (e < s.nev ? e : s.nev - 1);
   // the six coefficients (+1 / -1 / 0) arrive as ONE 8-byte constant load and become doubles by bit assembly: no
   // per-coefficient constant load and integer-to-double conversion on the critical path of the first phase
   const unsigned long long dw = *reinterpret_cast<const unsigned long long*>(&d);
@@ -238,7 +247,7 @@ template <class P, class T> __device__ __forceinline__ void run_momtab(const Sme
     const int cj = (int)(signed char)((dw >> (8 * j)) & 0xffull);
     const double c = __hiloint2double(cj == 0 ? 0 : (cj > 0 ? 0x3ff00000 : (int)0xbff00000), 0);
 #pragma unroll
-    for (int mu = 0; mu < 4; ++mu) q[mu] = fma(c, (double)s.ext[(e * P::NPAR + j) * 4 + mu], q[mu]);
+    for (int mu = 0; mu < 4; ++mu) q[mu] = fma(c, (double)__ldg(gm + (int64_t)(4 * j + mu) * s.ld), q[mu]);
   }
 #pragma unroll
   for (int mu = 0; mu < 4; ++mu) s.mom[(e * P::NMOM + m) * 4 + mu] = (T)q[mu];
@@ -261,20 +270,15 @@ __global__ void __launch_bounds__(P::NT, sizeof(T) == 8 ? P::MINB : P::MINB32) s
   const int tid = threadIdx.x;
   const int64_t ev0 = (int64_t)blockIdx.x * P::E;
 
-  // A5: momenta of the CTA's events (tail events re-read the last event and are not stored)
-  for (int i = tid; i < P::E * P::NPAR * 4; i += P::NT) {
-    const int e = i / (P::NPAR * 4), r = i - e * (P::NPAR * 4);
-    int64_t ge = ev0 + e;
-    if (ge >= n) ge = n - 1;
-    s.ext[i] = __ldg(mom + (int64_t)r * ld + ge);
-  }
+  // A5: the momenta are read straight from the caller's array by the tasks of step 0 (line momenta, external
+  // wavefunctions): no staging copy and no barrier in front of the first step
+  s.gmom = mom + ev0; s.ld = ld; s.nev = (int)((n - ev0) < (int64_t)P::E ? (n - ev0) : (int64_t)P::E);
   if (tid < 16) {
     unsigned long long w = 0;
 #pragma unroll
     for (int m = 0; m < 16; ++m) w |= (unsigned long long)pext(tid, m) << (4 * m);
-    s.pext4[tid] = w;
+    s.pext4[tid] = w;       // first read by the tasks of step 1, after the barrier that ends step 0
   }
-  __syncthreads();
 
   const int el = tid / P::NHEL, h = tid - el * P::NHEL;
   T me_h = P::template run<T>(s, tid, el, h, (T)k.mt);     // generated: producer steps + inner products + colour sum
