@@ -280,7 +280,12 @@ __global__ void __launch_bounds__(P::NT, sizeof(T) == 8 ? P::MINB : P::MINB32) s
     s.pext4[tid] = w;       // first read by the tasks of step 1, after the barrier that ends step 0
   }
 
-  const int el = tid / P::NHEL, h = tid - el * P::NHEL;
+  const int el = tid / P::NHEL, hl = tid - el * P::NHEL;
+  // helicity combination of this lane: bit i of the lane index is the helicity of particle HPERM[i] (a permutation
+  // chosen so that the lanes of a quarter warp share as many shared-memory operands as possible)
+  int h = 0;
+#pragma unroll
+  for (int i = 0; i < P::NPAR; ++i) h |= ((hl >> i) & 1) << ((P::HPERM >> (4 * i)) & 15);
   T me_h = P::template run<T>(s, tid, el, h, (T)k.mt);     // generated: producer steps + inner products + colour sum
 
   const int64_t ge = ev0 + el;
