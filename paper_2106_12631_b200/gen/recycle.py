@@ -87,6 +87,14 @@ class Closure:
         self.kind, self.a, self.b, self.flows = kind, a, b, flows   # kind: 'DOTS' row.col | 'DOTV' vector.vector
 
 
+def _closure_key(c):
+    """order of the closures inside a step: those sharing the second operand adjacent (it is loaded once)"""
+    mode = os.environ.get('MG_RC_CORDER', '0')
+    if mode == '4':
+        return (c.a.name, c.b.name)
+    return (c.b.name, c.a.name)
+
+
 class Program:
     def __init__(self, ng, chunk_budget=240):
         self.ng = ng
@@ -305,7 +313,7 @@ class Program:
                 else:
                     self.steps.append(("P", list(ps)))
             # closures sharing the second operand are adjacent: it is loaded once
-            self.steps.append(("F", sorted(ch, key=lambda c: (c.b.name, c.a.name))))
+            self.steps.append(("F", sorted(ch, key=_closure_key)))
         self._number()
         # HOIST: a producer step whose nodes can all be computed in an earlier producer step (operands born before it)
         # rides with that step when this costs no shared memory: one barrier-separated latency chain fewer
@@ -328,7 +336,7 @@ class Program:
                         merged = []
                         for k, it in trial:
                             if merged and k == "F" and merged[-1][0] == "F":
-                                merged[-1] = ("F", sorted(merged[-1][1] + it, key=lambda c: (c.b.name, c.a.name)))
+                                merged[-1] = ("F", sorted(merged[-1][1] + it, key=_closure_key))
                             else:
                                 merged.append((k, it))
                         keep = self.steps
