@@ -128,6 +128,7 @@ int mg_init_process(const mg_params* par, mg_process** out) {
   }
   DeviceGuard g(par->device);
   if (!g.ok || cudaStreamCreateWithFlags(&p->own_stream, cudaStreamNonBlocking) != cudaSuccess ||
+      cudaStreamCreateWithFlags(&p->own_stream2, cudaStreamNonBlocking) != cudaSuccess ||
       cudaEventCreate(&p->ev0) != cudaSuccess || cudaEventCreate(&p->ev1) != cudaSuccess) {
     cudaGetLastError(); delete p; return MG_ECUDA;
   }
@@ -143,6 +144,7 @@ int mg_free_process(mg_process* p) {
   if (p->ev0) cudaEventDestroy(p->ev0);
   if (p->ev1) cudaEventDestroy(p->ev1);
   if (p->own_stream) cudaStreamDestroy(p->own_stream);
+  if (p->own_stream2) cudaStreamDestroy(p->own_stream2);
   delete p;
   return MG_OK;
 }
@@ -345,16 +347,29 @@ int mg_sigmakin_host(mg_process* p, const void* h_momenta, int64_t n, int64_t ld
   const size_t me_off = (mom_b + 255) / 256 * 256;
   int rc = ensure_scratch(p, me_off + me_b, 0); if (rc != MG_OK) return rc;
   char* d = (char*)p->d_scratch;
-  cudaStream_t s = p->own_stream;
-  cudaError_t e = cudaMemcpyAsync(d, h_momenta, mom_b, cudaMemcpyHostToDevice, s);
-  if (e == cudaSuccess) e = cudaEventRecord(p->ev0, s);
-  MeArgs a{d, n, ld, d + me_off, nullptr, nullptr, nullptr, p->hel_mask};
-  if (e == cudaSuccess) e = launch_me(p, a, s);
-  if (e == cudaSuccess) e = cudaEventRecord(p->ev1, s);
-  if (e == cudaSuccess) e = cudaMemcpyAsync(h_me, d + me_off, me_b, cudaMemcpyDeviceToHost, s);
-  if (e == cudaSuccess) e = cudaStreamSynchronize(s);
+  // The batch goes through in chunks of events that alternate between two streams, so that the H2D copy of one chunk
+  // and the D2H copy of another overlap the kernel of a third (PAPER.md:112 copy:compute balance; the momenta are
+  // structure-of-arrays, so a chunk is a 2-D copy: `rows` rows of `width` events with row pitch ld).
+  const int64_t min_chunk = 1 << 16;
+  int nchunk = (int)(n / min_chunk); if (nchunk < 1) nchunk = 1; if (nchunk > 8) nchunk = 8;
+  const int64_t per = ((n + nchunk - 1) / nchunk + 31) / 32 * 32;
+  cudaStream_t st[2] = {p->own_stream, p->own_stream2};
+  cudaError_t e = cudaEventRecord(p->ev0, st[0]);
+  int c = 0;
+  for (int64_t c0 = 0; c0 < n && e == cudaSuccess; c0 += per, ++c) {
+    const int64_t width = (n - c0) < per ? (n - c0) : per;
+    cudaStream_t s = st[c & 1];
+    e = cudaMemcpy2DAsync(d + (size_t)c0 * es, (size_t)ld * es, (const char*)h_momenta + (size_t)c0 * es, (size_t)ld * es,
+                          (size_t)width * es, rows, cudaMemcpyHostToDevice, s);
+    MeArgs a{d + (size_t)c0 * es, width, ld, d + me_off + (size_t)c0 * es, nullptr, nullptr, nullptr, p->hel_mask};
+    if (e == cudaSuccess) e = launch_me(p, a, s);
+    if (e == cudaSuccess) e = cudaMemcpyAsync((char*)h_me + (size_t)c0 * es, d + me_off + (size_t)c0 * es, (size_t)width * es, cudaMemcpyDeviceToHost, s);
+  }
+  if (e == cudaSuccess) e = cudaStreamSynchronize(st[1]);
+  if (e == cudaSuccess) e = cudaEventRecord(p->ev1, st[0]);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(st[0]);
   if (e != cudaSuccess) { cudaGetLastError(); return MG_ECUDA; }
-  float ms = 0; cudaEventElapsedTime(&ms, p->ev0, p->ev1); p->last_kernel_ms = ms;
+  float ms = 0; cudaEventElapsedTime(&ms, p->ev0, p->ev1); p->last_kernel_ms = ms;     // whole pipelined call
   return MG_OK;
 }
 

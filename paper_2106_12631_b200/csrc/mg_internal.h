@@ -20,7 +20,7 @@ struct mg_process {
   size_t scratch_bytes;
   void* h_pinned;
   size_t pinned_bytes;
-  cudaStream_t own_stream;
+  cudaStream_t own_stream, own_stream2;   // host-buffer calls: chunks alternate between the two (copy/compute overlap)
   cudaEvent_t ev0, ev1;
   double last_kernel_ms;
 };
