@@ -154,7 +154,8 @@ int mg_sigmakin_per_helicity(mg_process* p, const void* d_momenta, int64_t n, in
 
 /* Host-buffer forms (the end-to-end path; "copy ... to the host").  Synchronous.
  * mg_sigmakin_host: copies h_momenta [4*n_external][ld] to the device, runs sigmaKin, copies
- * h_me[n] back.  mg_run_host: runs A1-A13 for events [first_event, first_event+n) on the device and
+ * h_me[n] back; batches of 2^17 events or more go through in up to 8 chunks on two streams of the handle so that
+ * the copies overlap the kernels (pinned host buffers are needed for that overlap).  mg_run_host: runs A1-A13 for events [first_event, first_event+n) on the device and
  * copies momenta (nullable), ps_weight (nullable) and me to the host.  Device scratch is grown
  * inside the handle on first use and reused. */
 int mg_sigmakin_host(mg_process* p, const void* h_momenta, int64_t n, int64_t ld, void* h_me);
