@@ -401,3 +401,40 @@ def test_fp32_error_profile(mg, process):
     if process == 0:
         me = P.sigmakin_fused(7, 0, 1 << 24)
         assert bool(torch.isfinite(me).all().item()) and bool((me > 0).all().item())
+
+
+# ----------------------------------------------------------------------------- BASELINE.json full sizes
+@pytest.mark.parametrize("process,prec,n,seed,nsample", [
+    (0, 0, 16384, 42, 16384), (0, 0, 1 << 24, 7, 4096), (0, 1, 1 << 24, 7, 4096),
+    (1, 0, 1 << 22, 7, 4096), (1, 1, 1 << 22, 7, 4096), (2, 0, 1 << 21, 7, 1024), (2, 1, 1 << 21, 7, 1024),
+    (3, 0, 1 << 20, 7, 256), (3, 1, 1 << 20, 7, 256)])
+def test_full_size_configs_sampled_parity(mg, process, prec, n, seed, nsample):
+    """The five configurations of BASELINE.json at their full sizes, in the launch configuration bench.py times
+    (mg_rng -> mg_rambo -> mg_filter_helicities -> mg_sigmakin with the event weight): a strided sample of events
+    covering the whole index range (first, last and ragged positions included) is compared with the oracle fed the
+    GPU's momenta; the whole batch must be finite and positive and its weights must satisfy w = W * ME (R18)."""
+    P = mg.Process(process, prec)
+    ld = mg.padded_stride(n)
+    rnd = P.rng(seed, 0, n)
+    mom, w = P.rambo(rnd, n)
+    del rnd
+    P.filter_helicities(mom, 32)
+    ew = torch.empty(ld, dtype=P.dtype, device=P.device)
+    me = P.sigmakin(mom, n, ps_weight=w, event_weight=ew)
+    assert bool(torch.isfinite(me[:n]).all().item()) and bool((me[:n] > 0).all().item())
+    assert torch.equal(ew[:n], w[:n] * me[:n])
+    idx = np.unique(np.concatenate([np.linspace(0, n - 1, nsample).astype(np.int64), [0, 1, 31, 32, n - 2, n - 1]]))
+    tidx = torch.from_numpy(idx).to(P.device)
+    mom_s = mom[:, tidx].cpu().numpy().astype(np.float64)
+    me_s = me[tidx].cpu().numpy().astype(np.float64)
+    me_o = oracle.me(process, soa_to_aos(mom_s, P.n_external))
+    rel = np.abs(me_s / me_o - 1)
+    print("full size process %d prec %d n %d: %d sampled events, max rel %.2e" % (process, prec, n, len(idx), rel.max()))
+    if prec == 0:
+        bad = rel > 1e-12
+        if bad.any():                     # ill-conditioned tail: decided by the long-double oracle (header of this file)
+            me_l = oracle.me(process, soa_to_aos(mom_s[:, bad], P.n_external), long_double=True)
+            assert (np.abs(me_o[bad] / me_l - 1) > 2.5e-13).all() and (np.abs(me_s[bad] / me_l - 1) < 1e-10).all()
+            assert bad.sum() <= max(1, len(idx) // 1000)
+    else:
+        assert rel.max() <= 1e-4
