@@ -20,6 +20,10 @@ namespace mg {
 struct Eemumu {
   static constexpr int NHEL = 16;
   static constexpr int NPAR = 4;
+#ifndef MG_EE_MINB
+#define MG_EE_MINB 6
+#endif
+  static constexpr int MINB = MG_EE_MINB;   // resident CTAs of 128 threads the register allocation aims at
   // Massless helicity spinors need three reals per particle (the "simplified" IXXXXX/OXXXXX of PAPER.md:136):
   //   omega_+ chi_+ = (a, b),  omega_+ chi_- = (-b^*, a),   a = sqrt(P+pz),  b = (px + i py)/sqrt(P+pz),
   // P+pz evaluated as pT^2/(P-pz) for pz < 0 (R19); along -z: a = 0, b = sqrt(2P) (B1).  One square root, one

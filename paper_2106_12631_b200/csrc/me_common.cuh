@@ -23,7 +23,7 @@ constexpr int kMeThreads = 128;
 //   static int    NHEL, NPAR
 // mask: good helicities (bit h).  me = norm * sum_h.  PER_HEL: write every helicity, ignore mask.
 template <class Proc, class T, bool PER_HEL>
-__global__ void __launch_bounds__(kMeThreads) sigmakin_kernel(Consts k, const T* __restrict__ mom, int64_t n, int64_t ld,
+__global__ void __launch_bounds__(kMeThreads, Proc::MINB) sigmakin_kernel(Consts k, const T* __restrict__ mom, int64_t n, int64_t ld,
                                                               T* __restrict__ me, const T* __restrict__ psw,
                                                               T* __restrict__ evw, T* __restrict__ hel_out, uint64_t mask) {
   const int64_t e = (int64_t)blockIdx.x * kMeThreads + threadIdx.x;

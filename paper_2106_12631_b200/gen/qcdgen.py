@@ -378,6 +378,7 @@ class Emitter:
         w("namespace mg {")
         w("struct %s {" % name)
         w("  static constexpr int NHEL = %d;" % (1 << npar))
+        w("  static constexpr int MINB = %d;   // resident CTAs of 128 threads the register allocation aims at" % int(os.environ.get("MG_TPE%d_MINB" % ng, {2: 3}.get(ng, 1))))
         w("  static constexpr int NPAR = %d;" % npar)
         w("  static constexpr int NFLOW = %d;" % nf)
         w("  static constexpr int NIK = %d;" % (len(self.gsets) + 1))
