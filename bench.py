@@ -36,6 +36,17 @@ PROC_NAME = {0: "e+ e- -> mu+ mu-", 1: "g g -> t t~", 2: "g g -> t t~ g", 3: "g 
 CPU_SAMPLE = {0: 1 << 19, 1: 1 << 19, 2: 1 << 16, 3: 1 << 12}
 # reference arm: events per step (a bounded sample so that steps+warmup end within minutes)
 REF_SAMPLE = {0: 1 << 17, 1: 1 << 17, 2: 1 << 13, 3: 1 << 9}
+# the kernel bench.py brackets with CUDA events for the roofline (what mg_sigmakin launches for that workload)
+KERNEL_NAME = {0: "mg::sigmakin_kernel<mg::Eemumu, %s, false>", 1: "mg::sigmakin_kernel<mg::Ggtt, %s, false>",
+               2: "mg::rc::sigmakin_recycle_kernel<mg::RcGgttg, %s, %s, 0>", 3: "mg::rc::sigmakin_recycle_kernel<mg::RcGgttgg, %s, %s, 0>"}
+
+
+def kernel_name(process, prec):
+    t = "double" if prec == 0 else "float"
+    name = KERNEL_NAME[process]
+    return name % ((t, t) if name.count("%s") == 2 else (t,))
+
+
 PAPER_BASELINE = {"ggttgg_fp64": 5e5, "eemumu_fp64": 1.37e9, "eemumu_fp32": 3.28e9}   # V100
 
 # FP64 / FP32 FMA lanes per SM; peak = 148 SMs x lanes x 2 x sm clock
@@ -83,13 +94,24 @@ class ClockSampler(threading.Thread):
 
 
 def cpu_baseline(process, seed, sample):
+    """The oracle as it stands on the host cores: the whole pipeline (the reported value), and its two legs timed
+    separately: Philox + RAMBO (single thread in the oracle's C API) and the matrix element (all threads)."""
     import oracle
     oracle.lib()
     t = time.perf_counter()
     oracle.pipeline(process, seed, 0, sample)
     dt = time.perf_counter() - t
+    t = time.perf_counter()
+    rho = oracle.uniforms(seed, 0, sample, oracle.N_FINAL[process])
+    mom, w, _ = oracle.rambo(rho, oracle.masses(process), 1500.0)
+    dt_gen = time.perf_counter() - t
+    t = time.perf_counter()
+    oracle.me(process, mom)
+    dt_me = time.perf_counter() - t
     return {"value": sample / dt, "unit": "MEs/s", "cores": oracle.hardware_threads(), "kind": "oracle",
-            "sample": "%d events of %s (Philox -> RAMBO -> ME), oracle FP64, %.1f s" % (sample, PROC_NAME[process], dt)}
+            "sample": "%d events of %s (Philox -> RAMBO -> ME), oracle FP64, %.1f s" % (sample, PROC_NAME[process], dt),
+            "legs": {"rng_rambo_events_per_s": sample / dt_gen, "rng_rambo_threads": 1,
+                     "me_events_per_s": sample / dt_me, "me_threads": oracle.hardware_threads()}}
 
 
 def run_reference(args):
@@ -182,7 +204,8 @@ def time_workload(mg, torch, name, device_index, steps, warmup, dist=None, sampl
     finite = bool(torch.isfinite(me[:n]).all().item())
     flops = P.flops_per_event(mg.STAGE_SIGMAKIN)
     step_bytes = n * (P.bytes_per_event(mg.STAGE_RNG) + P.bytes_per_event(mg.STAGE_RAMBO) + P.bytes_per_event(mg.STAGE_SIGMAKIN))
-    return {"P": P, "n": n, "ld": ld, "mask": mask, "total_ms": total_ms, "kern_ms": kern_ms, "mean_me": mean_me,
+    rescued = P.last_rescued() if (prec == 1 and process >= 2) else 0
+    return {"P": P, "n": n, "ld": ld, "mask": mask, "total_ms": total_ms, "kern_ms": kern_ms, "mean_me": mean_me, "rescued": rescued,
             "finite": finite, "flops_per_event": flops, "step_bytes": step_bytes, "process": process, "prec": prec,
             "seed": seed, "cfg": cfg, "world": world}
 
@@ -243,6 +266,49 @@ def stage_rates(mg, torch, r, reps=20):
     return out
 
 
+def small_batch_step(mg, torch, r, reps=200):
+    """Config 1 (16 384 events) is launch bound: microseconds per step of (a) the three launches, (b) the same three
+    launches replayed from a CUDA graph, (c) the one fused launch (mg_sigmakin_fused)."""
+    P, n, ld = r["P"], r["n"], r["ld"]
+    rnd = P.empty(4 * P.n_final, n, ld)
+    mom = P.empty(4 * P.n_external, n, ld)
+    w = torch.empty(ld, dtype=P.dtype, device=P.device)
+    me = torch.empty(ld, dtype=P.dtype, device=P.device)
+    ew = torch.empty(ld, dtype=P.dtype, device=P.device)
+
+    def three():
+        P.rng(r["seed"], 0, n, out=rnd)
+        P.rambo(rnd, n, mom, w)
+        P.sigmakin(mom, n, me, w, ew)
+
+    def timed(fn):
+        for _ in range(5):
+            fn()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        a.record()
+        for _ in range(reps):
+            fn()
+        b.record()
+        torch.cuda.synchronize()
+        return a.elapsed_time(b) / reps * 1e3
+
+    out = {"three_launches_us": timed(three), "fused_launch_us": timed(lambda: P.sigmakin_fused(r["seed"], 0, n, me, w, ew))}
+    try:
+        g = torch.cuda.CUDAGraph()
+        side = torch.cuda.Stream()
+        with torch.cuda.stream(side):
+            three()
+        torch.cuda.synchronize()
+        with torch.cuda.graph(g, stream=side):
+            three()
+        out["graph_replay_us"] = timed(g.replay)
+    except Exception as e:
+        out["graph_replay_us"] = "failed: %s" % e
+    out["events"] = n
+    return out
+
+
 def batch_sweep(mg, torch, name, device_index):
     """Throughput against the number of events per launch (PAPER.md:104 Fig. 5 and its two definitions, :156-164:
     kernel only, and kernel + device-to-host copy of the matrix elements)."""
@@ -279,8 +345,10 @@ def e2e_measure(mg, torch, r, steps):
     P, n, ld = r["P"], r["n"], r["ld"]
     h_mom = torch.empty((4 * P.n_external, ld), dtype=P.dtype).pin_memory()
     h_me = torch.empty(n, dtype=P.dtype).pin_memory()
-    P.run_host(r["seed"], 0, n, h_me, h_mom)           # fills the pinned host momenta (untimed)
+    h_ref = torch.empty(n, dtype=P.dtype).pin_memory()
+    P.run_host(r["seed"], 0, n, h_ref, h_mom)          # fills the pinned host momenta (untimed) and the MEs of one launch
     P.sigmakin_host(h_mom, n, h_me)                    # warm-up
+    assert torch.equal(h_me, h_ref), "chunked host call and single launch disagree"
     torch.cuda.synchronize()
     t = time.perf_counter()
     for _ in range(steps):
@@ -312,10 +380,22 @@ def main():
         run_reference(args)
         return
 
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        # one process per GPU: re-run this command under torchrun (the driver launches it that way itself for N > 1)
+        import socket
+        sock = socket.socket()
+        sock.bind(("127.0.0.1", 0))
+        port = sock.getsockname()[1]
+        sock.close()
+        os.environ.setdefault("NCCL_DEBUG", "INFO")          # the communicator log shows the ranks and the transport
+        os.execv(sys.executable, [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", str(args.gpus),
+                                  "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:])
     import torch
     import paper_2106_12631_b200 as mg
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device (there is no CPU fallback)")
+    if int(os.environ.get("WORLD_SIZE", "1")) != args.gpus:
+        raise SystemExit("bench.py --gpus %d was launched with WORLD_SIZE=%s" % (args.gpus, os.environ.get("WORLD_SIZE", "1")))
     dist = None
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
     if int(os.environ.get("WORLD_SIZE", "1")) > 1:
@@ -353,30 +433,40 @@ def main():
                    "l2": "inputs larger than L2: %.0f MB of rnd+momenta traffic per step, new event range every step" % (r["step_bytes"] / 1e6),
                    "paper_baseline": "V100, PAPER.md:116/:159 (context, other hardware)" if args.workload in PAPER_BASELINE else None},
         "e2e": e2e,
-        "gpu_launches": 3 * args.steps,
-        "roofline": {"bound": "alu", "kernel": "sigmakin_kernel", "achieved": achieved_tf, "peak": peak_tf, "unit": "TFLOP/s",
+        # rng, rambo, sigmaKin per step; FP32 handles of g g -> t t~ g (g) add the double-precision pass over the listed events
+        "gpu_launches": (4 if (prec == 1 and r["process"] >= 2) else 3) * args.steps,
+        "roofline": {"bound": "alu", "kernel": kernel_name(r["process"], prec), "achieved": achieved_tf, "peak": peak_tf, "unit": "TFLOP/s",
                      "frac": achieved_tf / peak_tf, "traffic": None,
                      "flops_per_event": r["flops_per_event"], "kernel_ms": r["kern_ms"],
+                     "peak_kind": "nominal (lanes x clock); the measured_* entries are on-box microbenchmarks of the same pipe",
                      "peak_source": "148 SMs x %d FMA lanes x 2 x %.0f MHz (MEASURED_PEAKS.json sm_max_mhz)" % (LANES[prec], sm_max)},
         "mean_me": r["mean_me"], "all_finite": r["finite"],
     }
     if rank == 0:
         out["clocks"] = sampler.result()
         try:
-            out["roofline"]["measured_fma_chain_tflops"] = mg.measure_alu_peak(prec, local_rank)
+            from paper_2106_12631_b200 import probe
+            out["roofline"]["measured_fma_chain_tflops"] = probe.alu_tflops(prec, local_rank, 0)
             # how the FMA is fed decides its rate on sm_100a: three distinct register operands vs tensor-core FP64
-            out["roofline"]["measured_fma_3reg_tflops"] = mg.measure_alu_mode(prec, local_rank, 1)
+            out["roofline"]["measured_fma_3reg_tflops"] = probe.alu_tflops(prec, local_rank, 1)
             if prec == 0:
-                out["roofline"]["measured_dmma_tflops"] = mg.measure_alu_mode(prec, local_rank, 2)
+                out["roofline"]["measured_dmma_tflops"] = probe.alu_tflops(prec, local_rank, 2)
         except Exception as e:
             out["roofline"]["measured_fma_chain_tflops"] = "failed: %s" % e
         try:
             out["stages"] = stage_rates(mg, torch, r)
         except Exception as e:
             out["stages"] = "failed: %s" % e
+        # DRAM bytes per launch of that kernel from a committed ncu --set full capture of this workload, if there is one
         tr = os.path.join(ROOT, "profiles", "traffic.json.txt")
-        if os.path.exists(tr):
-            out["roofline"]["traffic"] = json.load(open(tr)).get(args.workload)
+        ent = json.load(open(tr)).get(args.workload) if os.path.exists(tr) else None
+        if isinstance(ent, dict):
+            out["roofline"]["traffic"] = ent.get("bytes")
+            out["roofline"]["traffic_source"] = ent.get("source")
+        else:
+            out["roofline"]["traffic_source"] = "no ncu capture of this workload under profiles/"
+        if prec == 1 and r["process"] >= 2:
+            out["config"]["fp32_events_recomputed_in_double"] = r["rescued"]
     if rank == 0 and world == 1 and not args.no_extra:
         out["cpu_baseline"] = cpu_baseline(r["process"], r["seed"], CPU_SAMPLE[r["process"]])
         others = []
@@ -389,8 +479,13 @@ def main():
                 tf = o["flops_per_event"] * o["n"] / (o["kern_ms"] * 1e-3) / 1e12
                 others.append({"workload": name, "value": o["n"] * 3 / (o["total_ms"] * 1e-3), "unit": "MEs/s",
                                "sigmakin_MEs_per_s": o["n"] / (o["kern_ms"] * 1e-3), "sigmakin_ms": o["kern_ms"],
-                               "alu_frac": tf / pk, "flops_per_event": o["flops_per_event"], "mean_me": o["mean_me"],
+                               "kernel": kernel_name(o["process"], o["prec"]),
+                               "alu_frac_of_nominal": tf / pk, "flops_per_event": o["flops_per_event"], "mean_me": o["mean_me"],
                                "all_finite": o["finite"], "stages": stage_rates(mg, torch, o, reps=10)})
+                if o["prec"] == 1 and o["process"] >= 2:
+                    others[-1]["fp32_events_recomputed_in_double"] = o["rescued"]
+                if name == "eemumu_16k_fp64":
+                    others[-1]["small_batch"] = small_batch_step(mg, torch, o)
                 del o
                 torch.cuda.empty_cache()
             except Exception as e:

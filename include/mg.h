@@ -28,6 +28,13 @@
  *    n, ld, the launch shape or the stream.
  *  - There is no CPU fallback: every entry point that computes needs a CUDA device of compute
  *    capability 10.x and fails with MG_ECUDA otherwise.
+ *  - Streams and threads: a handle may be used with any stream, and with different streams in successive calls.
+ *    Calls that need device scratch (the host-buffer forms, mg_weight_sums*, mg_unweight*, and mg_sigmakin /
+ *    mg_sigmakin_fused of the FP32 handles of g g -> t t~ g (g)) take it from regions owned by the handle; each
+ *    region remembers the end of its last use with an event, the next user's stream waits for it, and a region is
+ *    only reallocated after its last user has finished.  Two calls on different streams that need the same region
+ *    are therefore serialised on the device, never corrupted.  A handle must not be used by two HOST threads at the
+ *    same time (no locking); use one handle per thread.
  */
 #ifndef MG_B200_H
 #define MG_B200_H
@@ -38,7 +45,7 @@
 extern "C" {
 #endif
 
-typedef struct mg_process mg_process; /* opaque; owns constant tables and small device scratch */
+typedef struct mg_process mg_process; /* opaque; owns constant tables, two streams and device scratch regions */
 
 enum { MG_EEMUMU = 0, MG_GGTT = 1, MG_GGTTG = 2, MG_GGTTGG = 3 };
 enum { MG_FP64 = 0, MG_FP32 = 1 };
@@ -103,12 +110,12 @@ int mg_generate(mg_process* p, uint64_t seed, uint64_t first_event, int64_t n, i
                 void* d_momenta, void* d_ps_weight, void* stream);
 
 /* A1-A13 fused (PAPER.md:112-118 copy:compute balance): random numbers, momenta and matrix
- * element of events first_event .. first_event+n-1 without the momenta ever being stored.  Writes me[n] and, if
- * non-NULL, ps_weight[n] and event_weight[n] = ps_weight * me (R18); uses the installed helicity mask.  e+e- ->
- * mu+mu- and g g -> t t~ run one kernel with everything in registers; the shared-memory kernels of g g -> t t~ g(g)
- * stage the momenta in a device scratch buffer owned by the handle (grown on first use: that call synchronises the
- * device; later calls are asynchronous on `stream`).  Same values as mg_generate + mg_sigmakin up to rounding of
- * contracted multiply-adds.  Errors: MG_EINVAL (NULL/misaligned d_me, bad handle, n < 0), MG_ENOMEM, MG_ECUDA. */
+ * element of events first_event .. first_event+n-1 without the momenta ever being stored: ONE launch for every
+ * process.  Writes me[n] and, if non-NULL, ps_weight[n] and event_weight[n] = ps_weight * me (R18); uses the
+ * installed helicity mask.  e+e- -> mu+mu- and g g -> t t~ keep everything in registers; in the shared-memory kernels
+ * of g g -> t t~ g(g) one thread per event of the CTA generates the momenta into shared memory before the first step.
+ * Asynchronous on `stream`.  Same values as mg_generate + mg_sigmakin up to rounding of contracted multiply-adds.
+ * Errors: MG_EINVAL (NULL/misaligned d_me, bad handle, n < 0), MG_ENOMEM, MG_ECUDA. */
 int mg_sigmakin_fused(mg_process* p, uint64_t seed, uint64_t first_event, int64_t n,
                       void* d_me, void* d_ps_weight, void* d_event_weight, void* stream);
 
@@ -125,10 +132,17 @@ int mg_sigmakin_fused(mg_process* p, uint64_t seed, uint64_t first_event, int64_
  * as in mg_rng (R28): the decision depends on the global event index only.  Writes the batch-relative indices of
  * the kept events in increasing order to d_kept_out[0 .. *h_count_out) (caller allocates n int64) — a stable stream
  * compaction, unique result.  Synchronous.  MG_EINVAL for w_max <= 0, NULL or misaligned pointers.
- * Both use a device scratch buffer owned by the handle (grown on first use). */
+ * Both use a device scratch region owned by the handle (grown on first use).
+ *
+ * The *_async forms do the same work and leave the results ON THE DEVICE: d_sums_out[3] doubles, d_count_out one
+ * int64 (caller-owned device memory, 8-byte aligned); no allocation once the scratch has its size, no host
+ * synchronisation: they can be chained behind mg_sigmakin on one stream or captured in a CUDA graph. */
 int mg_weight_sums(mg_process* p, const void* d_weights, int64_t n, double* h_sums_out, void* stream);
 int mg_unweight(mg_process* p, uint64_t seed, uint64_t first_event, const void* d_weights, int64_t n, double w_max,
                 int64_t* d_kept_out, int64_t* h_count_out, void* stream);
+int mg_weight_sums_async(mg_process* p, const void* d_weights, int64_t n, double* d_sums_out, void* stream);
+int mg_unweight_async(mg_process* p, uint64_t seed, uint64_t first_event, const void* d_weights, int64_t n, double w_max,
+                      int64_t* d_kept_out, int64_t* d_count_out, void* stream);
 
 /* A12: good-helicity filter (R16).  Evaluates every helicity combination on the
  * first probe_n events of d_momenta (1 <= probe_n <= n... the caller guarantees probe_n events are
@@ -145,6 +159,19 @@ int mg_get_helicity_mask(const mg_process* p, uint64_t* h_out_mask);
  * non-NULL also writes event_weight[e] = ps_weight[e] * me[e] (R18). */
 int mg_sigmakin(mg_process* p, const void* d_momenta, int64_t n, int64_t ld, void* d_me,
                 const void* d_ps_weight, void* d_event_weight, void* stream);
+
+/* Mixed precision of the FP32 handles of g g -> t t~ g and g g -> t t~ g g (§6: single
+ * precision "would require ... a better control of numeric instabilities").  The FP32 kernel evaluates
+ * every propagator denominator in double and lists the events whose largest |s / denominator| exceeds kappa_max (soft
+ * or collinear gluons: the gauge cancellations between diagrams then amplify FP32 rounding by ~sqrt(kappa)); a second
+ * launch recomputes the listed events in double from the SAME FP32 momenta and overwrites their me / event_weight.
+ * The decision depends on the event's momenta only, so results stay independent of batch shape and stream.
+ * kappa_max = 0 switches the second pass off (pure FP32).  Default 1000 (2 % of flat RAMBO g g -> t t~ g g events,
+ * 0.5 % of g g -> t t~ g).  No effect on FP64 handles and on the other processes.  mg_last_rescued returns the number of events the
+ * most recent mg_sigmakin / mg_sigmakin_fused / host call sent through the double pass (synchronises with it). */
+int mg_set_fp32_rescue(mg_process* p, double kappa_max);
+double mg_get_fp32_rescue(const mg_process* p);
+int mg_last_rescued(mg_process* p, int64_t* h_count_out);
 
 /* Diagnostic form of A5-A10: |M|^2 of EVERY helicity combination (mask ignored, no 1/denominator):
  * d_me_hel[h*ld + e].  Used by the filter and by the parity tests (per-helicity |M|^2 is
@@ -163,24 +190,15 @@ int mg_run_host(mg_process* p, uint64_t seed, uint64_t first_event, int64_t n, i
                 void* h_momenta, void* h_ps_weight, void* h_me);
 
 /* Algorithmic work per event of one stage: explicit
- * tallies emitted with the kernels; flops for MG_STAGE_SIGMAKIN are per event for the CURRENT
- * helicity mask (FMA = 2). */
+ * tallies emitted with the kernels (FMA = 2).  MG_STAGE_SIGMAKIN: e+e- -> mu+mu- and g g -> t t~ (one thread per
+ * event, helicity loop over the good helicities) count the CURRENT helicity mask; the shared-memory kernels of
+ * g g -> t t~ g (g) evaluate every helicity combination and only drop the masked ones from the sum, so their count
+ * does not depend on the mask. */
 int64_t mg_flops_per_event(const mg_process* p, int stage);
 int64_t mg_bytes_per_event(const mg_process* p, int stage);
-/* Duration in ms of the dominant kernel of the last mg_*_host call, measured with CUDA events on
- * the library's stream (0 if none). */
+/* GPU time in ms of the sigmaKin launches of the last mg_*_host call: CUDA events around the sigmaKin launch(es) of
+ * every chunk on its stream, summed over the chunks (copies and the event generation excluded; 0 if none). */
 double mg_last_kernel_ms(const mg_process* p);
-
-/* Measured FMA throughput of the plain FP64 / FP32 ALUs of `device` in TFLOP/s (FMA = 2): a
- * register-only chain microbenchmark (the denominator of the "alu" roofline).
- * Synchronous, takes ~0.1 s. */
-int mg_measure_alu_peak(int precision, int device, double* h_tflops_out);
-/* The same measurement for the three ways an FMA can be fed on sm_100a (SURVEY.md §8(d) asks for
- * the peak to be confirmed on the box): mode 0 = the chain of mg_measure_alu_peak (one register operand plus two
- * loop constants), mode 1 = three distinct register operands per FMA (what a product of two loaded wavefunctions
- * accumulates into), mode 2 = the FP64 tensor-core instruction mma.sync m8n8k4 (FP64 only, else MG_EINVAL).
- * Synchronous, ~0.1 s.  Errors as mg_measure_alu_peak. */
-int mg_measure_alu_mode(int precision, int device, int mode, double* h_tflops_out);
 
 const char* mg_strerror(int code);
 const char* mg_version(void);

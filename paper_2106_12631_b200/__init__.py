@@ -69,8 +69,11 @@ def lib():
         "mg_flops_per_event": (i64, [vp, C.c_int]),
         "mg_bytes_per_event": (i64, [vp, C.c_int]),
         "mg_last_kernel_ms": (C.c_double, [vp]),
-        "mg_measure_alu_peak": (C.c_int, [C.c_int, C.c_int, C.POINTER(C.c_double)]),
-        "mg_measure_alu_mode": (C.c_int, [C.c_int, C.c_int, C.c_int, C.POINTER(C.c_double)]),
+        "mg_weight_sums_async": (C.c_int, [vp, vp, i64, vp, vp]),
+        "mg_unweight_async": (C.c_int, [vp, u64, u64, vp, i64, C.c_double, vp, vp, vp]),
+        "mg_set_fp32_rescue": (C.c_int, [vp, C.c_double]),
+        "mg_get_fp32_rescue": (C.c_double, [vp]),
+        "mg_last_rescued": (C.c_int, [vp, C.POINTER(i64)]),
         "mg_strerror": (C.c_char_p, [C.c_int]),
         "mg_version": (C.c_char_p, []),
     }
@@ -86,7 +89,8 @@ EXPORTED = ["mg_default_params", "mg_init_process", "mg_free_process", "mg_n_ext
             "mg_padded_stride", "mg_rng_words", "mg_rng", "mg_rambo", "mg_generate", "mg_filter_helicities",
             "mg_set_helicity_mask", "mg_get_helicity_mask", "mg_sigmakin", "mg_sigmakin_per_helicity", "mg_sigmakin_fused", "mg_weight_sums", "mg_unweight",
             "mg_sigmakin_host", "mg_run_host", "mg_flops_per_event", "mg_bytes_per_event", "mg_last_kernel_ms",
-            "mg_measure_alu_peak", "mg_measure_alu_mode", "mg_strerror", "mg_version"]
+            "mg_weight_sums_async", "mg_unweight_async", "mg_set_fp32_rescue", "mg_get_fp32_rescue", "mg_last_rescued",
+            "mg_strerror", "mg_version"]
 
 
 def _check(rc):
@@ -105,20 +109,6 @@ def default_params(process, precision=FP64, device=0, **kw):
     for k, v in kw.items():
         setattr(p, k, v)
     return p
-
-
-def measure_alu_mode(precision=FP64, device=0, mode=0):
-    """TFLOP/s of mg_measure_alu_mode: 0 = FMA chain, 1 = three distinct register operands, 2 = FP64 mma.sync m8n8k4."""
-    v = C.c_double()
-    _check(lib().mg_measure_alu_mode(precision, device, mode, C.byref(v)))
-    return v.value
-
-
-def measure_alu_peak(precision=FP64, device=0):
-    """TFLOP/s of an FMA-chain microbenchmark on `device` (mg_measure_alu_peak)."""
-    v = C.c_double()
-    _check(lib().mg_measure_alu_peak(precision, device, C.byref(v)))
-    return v.value
 
 
 def _ptr(t):
@@ -236,6 +226,31 @@ class Process:
         cnt = C.c_int64()
         _check(lib().mg_unweight(self._h, seed, first_event, _ptr(weights), n, float(w_max), _ptr(kept), C.byref(cnt), _stream(self.device)))
         return kept[:cnt.value]
+
+    def weight_sums_async(self, weights, n, out=None):
+        """mg_weight_sums_async: (sum w, sum w^2, max w) left on the device (float64[3]); no host synchronisation."""
+        out = out if out is not None else torch.empty(3, dtype=torch.float64, device=self.device)
+        _check(lib().mg_weight_sums_async(self._h, _ptr(weights), n, _ptr(out), _stream(self.device)))
+        return out
+
+    def unweight_async(self, seed, first_event, weights, n, w_max, kept=None, count=None):
+        """mg_unweight_async: kept indices and their number (int64[1]) left on the device; no host synchronisation."""
+        kept = kept if kept is not None else torch.empty(max(n, 1), dtype=torch.int64, device=self.device)
+        count = count if count is not None else torch.empty(1, dtype=torch.int64, device=self.device)
+        _check(lib().mg_unweight_async(self._h, seed, first_event, _ptr(weights), n, float(w_max), _ptr(kept), _ptr(count), _stream(self.device)))
+        return kept, count
+
+    # ---- mixed precision of the FP32 handles of g g -> t t~ g (g)
+    def set_fp32_rescue(self, kappa_max):
+        _check(lib().mg_set_fp32_rescue(self._h, float(kappa_max)))
+
+    def fp32_rescue(self):
+        return float(lib().mg_get_fp32_rescue(self._h))
+
+    def last_rescued(self):
+        c = C.c_int64()
+        _check(lib().mg_last_rescued(self._h, C.byref(c)))
+        return c.value
 
     # ---- host-buffer (end-to-end) forms; tensors are CPU tensors (pinned for speed)
     def sigmakin_host(self, h_momenta, n, h_me):

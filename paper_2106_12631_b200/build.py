@@ -1,8 +1,9 @@
-"""In-tree build of libmg_b200.so with nvcc for sm_100a (cross-compiles without a GPU).
+"""In-tree build with nvcc for sm_100a (cross-compiles without a GPU).
 
-    python -m paper_2106_12631_b200.build [--force]
+    python -m paper_2106_12631_b200.build [--force] [-v]
 
-One object per .cu (compiled in parallel), linked into paper_2106_12631_b200/libmg_b200.so.
+One object per .cu (compiled in parallel), linked into paper_2106_12631_b200/libmg_b200.so (the product, include/mg.h)
+and paper_2106_12631_b200/libmg_probe.so (the ALU microbenchmarks bench.py prints, include/mg_probe.h).
 """
 import concurrent.futures
 import os
@@ -13,9 +14,11 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libmg_b200.so")
-SOURCES = ["mg_api.cu", "rng_rambo.cu", "me_eemumu.cu", "me_ggtt.cu", "me_ggttg.cu", "me_ggttgg.cu", "me_tables.cu", "alu_peak.cu", "xsec.cu"]
+PROBE_LIB = os.path.join(HERE, "libmg_probe.so")
+SOURCES = ["mg_api.cu", "rng_rambo.cu", "me_eemumu.cu", "me_ggtt.cu", "me_ggttg.cu", "me_ggttgg.cu", "me_tables.cu", "xsec.cu"]
+PROBE_SOURCES = ["alu_peak.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
-              "-Xcompiler", "-fPIC", "-Xptxas", "-v", "--fmad=true"] + os.environ.get("MG_NVCC_EXTRA", "").split()
+              "-Xcompiler", "-fPIC", "-Xptxas", "-v", "--fmad=true"]
 
 
 def _newest_header():
@@ -41,15 +44,18 @@ def _compile(src, force, hdr_time):
 def build(force=False, verbose=False):
     os.makedirs(OBJ, exist_ok=True)
     hdr_time = _newest_header()
-    with concurrent.futures.ThreadPoolExecutor(max_workers=len(SOURCES)) as ex:
-        results = list(ex.map(lambda s: _compile(s, force, hdr_time), SOURCES))
+    srcs = SOURCES + PROBE_SOURCES
+    with concurrent.futures.ThreadPoolExecutor(max_workers=len(srcs)) as ex:
+        results = list(ex.map(lambda s: _compile(s, force, hdr_time), srcs))
     objs = [o for o, _ in results]
     log = "".join(l for _, l in results)
     if log:
-        with open(os.path.join(OBJ, "ptxas.log"), "w") as f:
+        with open(os.path.join(OBJ, "ptxas.log"), "a") as f:
             f.write(log)
-    if force or not os.path.exists(LIB) or any(os.path.getmtime(o) > os.path.getmtime(LIB) for o in objs):
-        subprocess.check_call(["nvcc", "-shared", "-cudart", "static", "-o", LIB] + objs)
+    for lib, n0, n1 in ((LIB, 0, len(SOURCES)), (PROBE_LIB, len(SOURCES), len(srcs))):
+        o = objs[n0:n1]
+        if force or not os.path.exists(lib) or any(os.path.getmtime(x) > os.path.getmtime(lib) for x in o):
+            subprocess.check_call(["nvcc", "-gencode", "arch=compute_100a,code=sm_100a", "-shared", "-cudart", "shared", "-Xlinker", "-rpath=/usr/local/cuda/lib64", "-o", lib] + o)
     if verbose and log:
         print(log)
     return LIB

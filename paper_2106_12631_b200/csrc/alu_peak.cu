@@ -1,7 +1,8 @@
-// alu_peak.cu — FMA-chain microbenchmark behind mg_measure_alu_peak(): the measured denominator of
-// the "alu" roofline ("confirm with a DFMA/FFMA-chain microbenchmark on the box").
-// Every thread runs 16 independent accumulator chains of a*x+b; nothing is read from memory.
-#include "mg_internal.h"
+// alu_peak.cu — FMA microbenchmarks behind include/mg_probe.h (libmg_probe.so, NOT part of the product library):
+// the measured denominators of the "alu" roofline ("confirm with a DFMA/FFMA-chain microbenchmark
+// on the box").  Every thread runs independent accumulator chains; nothing is read from memory.
+#include <cuda_runtime.h>
+#include "../../include/mg_probe.h"
 
 namespace mg {
 namespace {
@@ -126,9 +127,21 @@ cudaError_t measure_alu_peak(int precision, int device, int mode, double* tflops
   cudaDeviceProp prop;
   cudaError_t e = cudaGetDeviceProperties(&prop, device);
   if (e != cudaSuccess) return e;
-  if (mode == 1) return precision == MG_FP64 ? run_mode<double>(prop.multiProcessorCount, 1, tflops) : run_mode<float>(prop.multiProcessorCount, 1, tflops);
+  if (mode == 1) return precision == 0 ? run_mode<double>(prop.multiProcessorCount, 1, tflops) : run_mode<float>(prop.multiProcessorCount, 1, tflops);
   if (mode == 2) return run_mode<double>(prop.multiProcessorCount, 2, tflops);
-  return precision == MG_FP64 ? run<double>(prop.multiProcessorCount, tflops) : run<float>(prop.multiProcessorCount, tflops);
+  return precision == 0 ? run<double>(prop.multiProcessorCount, tflops) : run<float>(prop.multiProcessorCount, tflops);
 }
 
 }  // namespace mg
+
+extern "C" int mg_probe_alu(int precision, int device, int mode, double* h_tflops_out) {
+  if (!h_tflops_out || device < 0 || (precision != 0 && precision != 1) || mode < 0 || mode > 2) return -1;
+  if (mode == 2 && precision != 0) return -1;
+  int ndev = 0, prev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || device >= ndev) { cudaGetLastError(); return -3; }
+  cudaGetDevice(&prev);
+  cudaSetDevice(device);
+  const cudaError_t e = mg::measure_alu_peak(precision, device, mode, h_tflops_out);
+  cudaSetDevice(prev);
+  return e == cudaSuccess ? 0 : -3;
+}

@@ -76,17 +76,28 @@ template <class T> MG_HD Chi<T> chi(Mom<T> p, T P, int lambda) {
   return x;
 }
 
-// omega_+ = sqrt(E+P), omega_- = sqrt(E-P) = m/omega_+ (exactly 0 for m = 0).  For m = 0 the energy
-// is taken as |p| (not the stored E), so that the spinor solves the Dirac equation of the 3-momentum
-// exactly even when the event generator left E and |p| a few ulps (or gamma^2 ulps) apart.
+// omega_+ = sqrt(E+P), omega_- = sqrt(E-P).  For m = 0 the energy is taken as |p| (not the stored E): omega_- is
+// exactly 0 and the spinor solves the Dirac equation of the 3-momentum exactly even when the event generator left E
+// and |p| a few ulps apart.  For m > 0 the pair is evaluated as
+//     omega_+- = ((E+m) +- P) / sqrt(2 (E+m)),
+// which equals sqrt(E +- P) on the mass shell and has no cancellation (E + m - P >= m).  Off the mass shell by
+// rounding (momenta stored in FP32: E^2 - P^2 - m^2 ~ 1e-7 E^2) sqrt(E+P) and m/sqrt(E+P) would be a different
+// function of (E, p, m) than the textbook u = (sqrt(E+m) chi, lambda P/sqrt(E+m) chi) of the plain definition
+// (omega_- differs by ~1e-7 E^2/m^2), and the gauge cancellations of soft and collinear events amplify that
+// difference; this form is the chiral rotation of the textbook spinor, term by term.
+template <class T> MG_HD void omegas(T E, T P, T m, T& wp, T& wm) {
+  if (m == (T)0) { wp = sqrt_<T>(P + P); wm = (T)0; return; }
+  const T em = E + m;
+  const T inv = rsqrt_<T>(em + em);
+  wp = (em + P) * inv; wm = (em - P) * inv;
+}
 // u(p,l)    = (omega_{-l} chi_l ; omega_{l} chi_l)            incoming fermion   (IXXXXX)
 // v(p,l)    = (omega_{l} chi_{-l} ; -omega_{-l} chi_{-l})     outgoing antifermion (IXXXXX)
 // ubar, vbar = psi^dagger gamma^0 = (psi_R^dagger | psi_L^dagger)   outgoing fermion / incoming antifermion (OXXXXX)
 template <class T> MG_HD Spinor<T> spinor_u(Mom<T> p, T m, int lambda) {
   const T P = sqrt_<T>(fma_<T>(p.v[1], p.v[1], fma_<T>(p.v[2], p.v[2], p.v[3] * p.v[3])));
-  const T ep = (m == (T)0 ? P : p.v[0]) + P;
-  const T iw = rsqrt_<T>(ep);
-  const T wp = ep * iw, wm = m * iw;
+  T wp, wm;
+  omegas<T>(p.v[0], P, m, wp, wm);
   const Chi<T> x = chi<T>(p, P, lambda);
   const T wl = lambda > 0 ? wm : wp, wr = lambda > 0 ? wp : wm;
   Spinor<T> s;
@@ -96,9 +107,8 @@ template <class T> MG_HD Spinor<T> spinor_u(Mom<T> p, T m, int lambda) {
 }
 template <class T> MG_HD Spinor<T> spinor_v(Mom<T> p, T m, int lambda) {
   const T P = sqrt_<T>(fma_<T>(p.v[1], p.v[1], fma_<T>(p.v[2], p.v[2], p.v[3] * p.v[3])));
-  const T ep = (m == (T)0 ? P : p.v[0]) + P;
-  const T iw = rsqrt_<T>(ep);
-  const T wp = ep * iw, wm = m * iw;
+  T wp, wm;
+  omegas<T>(p.v[0], P, m, wp, wm);
   const Chi<T> x = chi<T>(p, P, -lambda);
   const T wl = lambda > 0 ? wp : wm, wr = lambda > 0 ? -wm : -wp;
   Spinor<T> s;

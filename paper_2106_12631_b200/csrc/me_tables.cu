@@ -35,12 +35,7 @@ int64_t me_flops_per_event_fixed(int process) {
 int64_t me_flops_per_event_recycle(int process) {
   switch (process) {
     case MG_GGTTGG: return kFlopsRecycle_4;
-#ifndef MG_GGTTG_THREAD_PER_EVENT
     case MG_GGTTG: return kFlopsRecycle_3;
-#endif
-#ifdef MG_GGTT_RECYCLE
-    case MG_GGTT: return kFlopsRecycle_2;
-#endif
   }
   return -1;
 }

@@ -18,6 +18,10 @@ const ProcInfo kInfo[4] = {
     {6, 4, 64, 24, 123, 159, 512}, // gg -> tt~gg        (configs[4])
 };
 
+// FP32 handles of g g -> t t~ g (g): events with max |s / propagator denominator| above this go through the
+// double-precision pass (mg_set_fp32_rescue, chosen from profiles/r02_fp32_accuracy.md)
+const double kDefaultRescueKappa = 1000.0;
+
 inline bool valid_handle(const mg_process* p) { return p != nullptr; }
 inline size_t elem(const mg_process* p) { return p->par.precision == MG_FP64 ? 8 : 4; }
 inline bool aligned(const void* q, size_t a) { return ((uintptr_t)q % a) == 0; }
@@ -41,16 +45,46 @@ double rambo_w0(int n, double sqrt_s) {  // (pi/2)^(n-1) s^(n-2) / ((n-1)!(n-2)!
   return w;
 }
 
-int ensure_scratch(mg_process* p, size_t dev_bytes, size_t host_bytes) {
-  if (dev_bytes > p->scratch_bytes) {
-    if (p->d_scratch) cudaFree(p->d_scratch);
-    p->d_scratch = nullptr; p->scratch_bytes = 0;
-    cudaError_t e = cudaMalloc(&p->d_scratch, dev_bytes);
-    if (e != cudaSuccess) { cudaGetLastError(); return MG_ENOMEM; }
-    p->scratch_bytes = dev_bytes;
+// Scratch regions (mg_internal.h).  acquire(): the region holds >= bytes and everything `stream` does from here on
+// runs after the previous user of the region (on whatever stream) has finished; growing waits for that user on the
+// host before the old buffer is freed.  release(): marks the end of this use on `stream`.
+int acquire(mg_scratch& sc, size_t bytes, cudaStream_t stream) {
+  if (bytes > sc.bytes) {
+    if (sc.used && cudaEventSynchronize(sc.done) != cudaSuccess) { cudaGetLastError(); return MG_ECUDA; }
+    if (sc.d) cudaFree(sc.d);
+    sc.d = nullptr; sc.bytes = 0; sc.used = false;
+    const size_t want = bytes + bytes / 4;                      // head room: a slightly larger batch does not reallocate
+    if (cudaMalloc(&sc.d, want) != cudaSuccess) { cudaGetLastError(); return MG_ENOMEM; }
+    sc.bytes = want;
+  } else if (sc.used) {
+    if (cudaStreamWaitEvent(stream, sc.done, 0) != cudaSuccess) { cudaGetLastError(); return MG_ECUDA; }
   }
-  (void)host_bytes;
   return MG_OK;
+}
+int release(mg_scratch& sc, cudaStream_t stream) {
+  if (cudaEventRecord(sc.done, stream) != cudaSuccess) { cudaGetLastError(); return MG_ECUDA; }
+  sc.used = true;
+  return MG_OK;
+}
+bool scratch_init(mg_scratch& sc) {
+  sc.d = nullptr; sc.bytes = 0; sc.used = false;
+  return cudaEventCreateWithFlags(&sc.done, cudaEventDisableTiming) == cudaSuccess;
+}
+void scratch_free(mg_scratch& sc) {
+  if (sc.used) cudaEventSynchronize(sc.done);
+  if (sc.d) cudaFree(sc.d);
+  if (sc.done) cudaEventDestroy(sc.done);
+}
+
+// processes evaluated by the shared-memory kernels (recycle.cuh)
+inline bool shared_memory_kernel(const mg_process* p) { return p->par.process == MG_GGTTG || p->par.process == MG_GGTTGG; }
+// list of ill-conditioned events of an FP32 batch: [count (8 B, padded to 256)] [n event indices]
+inline bool wants_rescue(const mg_process* p) { return shared_memory_kernel(p) && p->par.precision == MG_FP32 && p->rescue_kappa > 0; }
+inline size_t rescue_bytes(int64_t n) { return 256 + (size_t)n * sizeof(int64_t); }
+inline void set_rescue(const mg_process* p, MeArgs& a, void* region) {
+  a.rescue_count = (unsigned long long*)region;
+  a.rescue_list = (int64_t*)((char*)region + 256);
+  a.rescue_kappa = p->rescue_kappa;
 }
 
 cudaError_t launch_me(const mg_process* p, const MeArgs& a, cudaStream_t s) {
@@ -61,6 +95,18 @@ cudaError_t launch_me(const mg_process* p, const MeArgs& a, cudaStream_t s) {
     case MG_GGTTGG: return launch_me_ggttgg(p, a, s);
   }
   return cudaErrorInvalidValue;
+}
+
+// launch_me plus, for FP32 handles of the shared-memory kernels, the list of ill-conditioned events in rescue region `slot`
+int run_me(mg_process* p, MeArgs& a, cudaStream_t s, int slot) {
+  if (!wants_rescue(p) || a.hel_out) return cuda_rc(launch_me(p, a, s));
+  mg_scratch& sc = p->sc_rescue[slot];
+  p->rescue_last_mask |= 1 << slot;
+  int rc = acquire(sc, rescue_bytes(a.n), s); if (rc != MG_OK) return rc;
+  set_rescue(p, a, sc.d);
+  const cudaError_t e = launch_me(p, a, s);
+  rc = release(sc, s);
+  return e != cudaSuccess ? cuda_rc(e) : rc;
 }
 
 int check_soa(const mg_process* p, const void* ptr, int64_t n, int64_t ld) {
@@ -126,12 +172,15 @@ int mg_init_process(const mg_params* par, mg_process** out) {
     const int ng = I.n_ext - 2;
     k.me_norm = pow(4 * pi * par->alpha_s, ng) / I.denom;                              // g_s^(2 n_g) / denominator
   }
+  p->sm_count = prop.multiProcessorCount;
+  p->rescue_kappa = kDefaultRescueKappa;
   DeviceGuard g(par->device);
-  if (!g.ok || cudaStreamCreateWithFlags(&p->own_stream, cudaStreamNonBlocking) != cudaSuccess ||
-      cudaStreamCreateWithFlags(&p->own_stream2, cudaStreamNonBlocking) != cudaSuccess ||
-      cudaEventCreate(&p->ev0) != cudaSuccess || cudaEventCreate(&p->ev1) != cudaSuccess) {
-    cudaGetLastError(); delete p; return MG_ECUDA;
-  }
+  bool ok = g.ok && cudaStreamCreateWithFlags(&p->own_stream, cudaStreamNonBlocking) == cudaSuccess &&
+            cudaStreamCreateWithFlags(&p->own_stream2, cudaStreamNonBlocking) == cudaSuccess &&
+            cudaEventCreate(&p->ev0) == cudaSuccess && cudaEventCreate(&p->ev1) == cudaSuccess &&
+            scratch_init(p->sc_host) && scratch_init(p->sc_xsec) && scratch_init(p->sc_rescue[0]) && scratch_init(p->sc_rescue[1]);
+  for (int i = 0; ok && i < 16; ++i) ok = cudaEventCreate(&p->kev[i]) == cudaSuccess;
+  if (!ok) { cudaGetLastError(); mg_free_process(p); return MG_ECUDA; }
   *out = p;
   return MG_OK;
 }
@@ -139,8 +188,8 @@ int mg_init_process(const mg_params* par, mg_process** out) {
 int mg_free_process(mg_process* p) {
   if (!p) return MG_OK;
   DeviceGuard g(p->par.device);
-  if (p->d_scratch) cudaFree(p->d_scratch);
-  if (p->h_pinned) cudaFreeHost(p->h_pinned);
+  scratch_free(p->sc_host); scratch_free(p->sc_xsec); scratch_free(p->sc_rescue[0]); scratch_free(p->sc_rescue[1]);
+  for (int i = 0; i < 16; ++i) if (p->kev[i]) cudaEventDestroy(p->kev[i]);
   if (p->ev0) cudaEventDestroy(p->ev0);
   if (p->ev1) cudaEventDestroy(p->ev1);
   if (p->own_stream) cudaStreamDestroy(p->own_stream);
@@ -203,7 +252,8 @@ int mg_sigmakin(mg_process* p, const void* d_momenta, int64_t n, int64_t ld, voi
   MeArgs a{d_momenta, n, ld, d_me, nullptr, nullptr, nullptr, p->hel_mask};
   if (d_ps_weight && d_event_weight) { a.psw = d_ps_weight; a.evw = d_event_weight; }
   DeviceGuard g(p->par.device); if (!g.ok) return MG_ECUDA;
-  return cuda_rc(launch_me(p, a, (cudaStream_t)stream));
+  p->rescue_last_mask = 0;
+  return run_me(p, a, (cudaStream_t)stream, 0);
 }
 
 int mg_sigmakin_fused(mg_process* p, uint64_t seed, uint64_t first_event, int64_t n, void* d_me, void* d_ps_weight, void* d_event_weight, void* stream) {
@@ -215,17 +265,24 @@ int mg_sigmakin_fused(mg_process* p, uint64_t seed, uint64_t first_event, int64_
   cudaStream_t s = (cudaStream_t)stream;
   if (p->par.process == MG_EEMUMU) return cuda_rc(launch_fused_eemumu(p, seed, first_event, n, d_me, d_ps_weight, d_event_weight, s));
   if (p->par.process == MG_GGTT) return cuda_rc(launch_fused_ggtt(p, seed, first_event, n, d_me, d_ps_weight, d_event_weight, s));
-  // shared-memory recycling kernels: momenta go through the handle's scratch buffer (< 1 % of their time)
-  const int64_t ld = (n + 31) / 32 * 32;
-  const size_t mom_b = (size_t)4 * p->n_ext * ld * es, w_b = (size_t)ld * es;
-  int rc = ensure_scratch(p, mom_b + w_b, 0); if (rc != MG_OK) return rc;
-  char* d = (char*)p->d_scratch;
-  void* d_w = d_ps_weight ? d_ps_weight : (void*)(d + mom_b);
-  cudaError_t e = launch_generate(p, seed, first_event, n, ld, d, d_w, s);
-  if (e != cudaSuccess) return cuda_rc(e);
-  MeArgs a{d, n, ld, d_me, nullptr, nullptr, nullptr, p->hel_mask};
-  if (d_event_weight) { a.psw = d_w; a.evw = d_event_weight; }
-  return cuda_rc(launch_me(p, a, s));
+  // shared-memory kernels: the CTA generates the momenta of its events into shared memory (recycle.cuh, M_GEN)
+  MeArgs a{nullptr, n, n, d_me, nullptr, d_event_weight, nullptr, p->hel_mask};
+  a.gen = true; a.seed = seed; a.first = first_event; a.psw_out = d_ps_weight;
+  p->rescue_last_mask = 0;
+  return run_me(p, a, s, 0);
+}
+
+int mg_weight_sums_async(mg_process* p, const void* d_weights, int64_t n, double* d_sums_out, void* stream) {
+  if (!valid_handle(p) || n < 0 || !d_sums_out || !aligned(d_sums_out, sizeof(double))) return MG_EINVAL;
+  DeviceGuard g(p->par.device); if (!g.ok) return MG_ECUDA;
+  cudaStream_t s = (cudaStream_t)stream;
+  if (n == 0) return cuda_rc(cudaMemsetAsync(d_sums_out, 0, 3 * sizeof(double), s));
+  if (!d_weights || !aligned(d_weights, elem(p))) return MG_EINVAL;
+  const int64_t nb = weight_sums_blocks(n);
+  int rc = acquire(p->sc_xsec, (size_t)nb * 3 * sizeof(double), s); if (rc != MG_OK) return rc;
+  const cudaError_t e = launch_weight_sums(p, d_weights, n, (double*)p->sc_xsec.d, d_sums_out, s);
+  rc = release(p->sc_xsec, s);
+  return e != cudaSuccess ? cuda_rc(e) : rc;
 }
 
 int mg_weight_sums(mg_process* p, const void* d_weights, int64_t n, double* h_sums_out, void* stream) {
@@ -236,18 +293,28 @@ int mg_weight_sums(mg_process* p, const void* d_weights, int64_t n, double* h_su
   DeviceGuard g(p->par.device); if (!g.ok) return MG_ECUDA;
   cudaStream_t s = (cudaStream_t)stream;
   const int64_t nb = weight_sums_blocks(n);
-  int rc = ensure_scratch(p, (size_t)nb * 3 * sizeof(double), 0); if (rc != MG_OK) return rc;
-  double* h = (double*)malloc((size_t)nb * 3 * sizeof(double));
-  if (!h) return MG_ENOMEM;
-  cudaError_t e = launch_weight_sums(p, d_weights, n, (double*)p->d_scratch, s);
-  if (e == cudaSuccess) e = cudaMemcpyAsync(h, p->d_scratch, (size_t)nb * 3 * sizeof(double), cudaMemcpyDeviceToHost, s);
+  int rc = acquire(p->sc_xsec, (size_t)(nb + 1) * 3 * sizeof(double), s); if (rc != MG_OK) return rc;
+  double* d_part = (double*)p->sc_xsec.d;
+  double* d_out = d_part + 3 * nb;
+  cudaError_t e = launch_weight_sums(p, d_weights, n, d_part, d_out, s);
+  if (e == cudaSuccess) e = cudaMemcpyAsync(h_sums_out, d_out, 3 * sizeof(double), cudaMemcpyDeviceToHost, s);
+  rc = release(p->sc_xsec, s);
   if (e == cudaSuccess) e = cudaStreamSynchronize(s);
-  if (e != cudaSuccess) { free(h); return cuda_rc(e); }
-  double s1 = 0, s2 = 0, mx = 0;
-  for (int64_t b = 0; b < nb; ++b) { s1 += h[3 * b]; s2 += h[3 * b + 1]; mx = h[3 * b + 2] > mx ? h[3 * b + 2] : mx; }   // block order: deterministic
-  free(h);
-  h_sums_out[0] = s1; h_sums_out[1] = s2; h_sums_out[2] = mx;
-  return MG_OK;
+  return e != cudaSuccess ? cuda_rc(e) : rc;
+}
+
+int mg_unweight_async(mg_process* p, uint64_t seed, uint64_t first_event, const void* d_weights, int64_t n, double w_max,
+                      int64_t* d_kept_out, int64_t* d_count_out, void* stream) {
+  if (!valid_handle(p) || n < 0 || !d_count_out || !aligned(d_count_out, sizeof(int64_t))) return MG_EINVAL;
+  DeviceGuard g(p->par.device); if (!g.ok) return MG_ECUDA;
+  cudaStream_t s = (cudaStream_t)stream;
+  if (n == 0) return cuda_rc(cudaMemsetAsync(d_count_out, 0, sizeof(int64_t), s));
+  if (!d_weights || !aligned(d_weights, elem(p)) || !d_kept_out || !aligned(d_kept_out, sizeof(int64_t)) || !(w_max > 0.0)) return MG_EINVAL;
+  const int64_t nt = unweight_tiles(n);
+  int rc = acquire(p->sc_xsec, (size_t)(nt + 1) * sizeof(unsigned long long), s); if (rc != MG_OK) return rc;
+  const cudaError_t e = launch_unweight(p, seed, first_event, d_weights, n, w_max, (unsigned long long*)p->sc_xsec.d, d_kept_out, d_count_out, s);
+  rc = release(p->sc_xsec, s);
+  return e != cudaSuccess ? cuda_rc(e) : rc;
 }
 
 int mg_unweight(mg_process* p, uint64_t seed, uint64_t first_event, const void* d_weights, int64_t n, double w_max,
@@ -259,18 +326,17 @@ int mg_unweight(mg_process* p, uint64_t seed, uint64_t first_event, const void* 
   DeviceGuard g(p->par.device); if (!g.ok) return MG_ECUDA;
   cudaStream_t s = (cudaStream_t)stream;
   const int64_t nt = unweight_tiles(n);
-  const size_t off_b = (size_t)(nt + 1) * sizeof(int64_t), cnt_b = (size_t)nt * sizeof(int);
-  int rc = ensure_scratch(p, off_b + cnt_b + (size_t)nt * 32 * sizeof(unsigned), 0); if (rc != MG_OK) return rc;
-  int64_t* d_off = (int64_t*)p->d_scratch;
-  int* d_cnt = (int*)((char*)p->d_scratch + off_b);
-  unsigned* d_bal = (unsigned*)((char*)p->d_scratch + off_b + cnt_b);
-  cudaError_t e = launch_unweight(p, seed, first_event, d_weights, n, w_max, d_cnt, d_bal, d_off, d_kept_out, s);
+  const size_t state_b = ((size_t)(nt + 1) * sizeof(unsigned long long) + 255) / 256 * 256;
+  int rc = acquire(p->sc_xsec, state_b + sizeof(int64_t), s); if (rc != MG_OK) return rc;
+  int64_t* d_count = (int64_t*)((char*)p->sc_xsec.d + state_b);
+  cudaError_t e = launch_unweight(p, seed, first_event, d_weights, n, w_max, (unsigned long long*)p->sc_xsec.d, d_kept_out, d_count, s);
   int64_t total = 0;
-  if (e == cudaSuccess) e = cudaMemcpyAsync(&total, d_off + nt, sizeof(int64_t), cudaMemcpyDeviceToHost, s);
+  if (e == cudaSuccess) e = cudaMemcpyAsync(&total, d_count, sizeof(int64_t), cudaMemcpyDeviceToHost, s);
+  rc = release(p->sc_xsec, s);
   if (e == cudaSuccess) e = cudaStreamSynchronize(s);
   if (e != cudaSuccess) return cuda_rc(e);
   *h_count_out = total;
-  return MG_OK;
+  return rc;
 }
 
 int mg_sigmakin_per_helicity(mg_process* p, const void* d_momenta, int64_t n, int64_t ld, void* d_me_hel, void* stream) {
@@ -345,31 +411,39 @@ int mg_sigmakin_host(mg_process* p, const void* h_momenta, int64_t n, int64_t ld
   const int rows = 4 * p->n_ext;
   const size_t mom_b = (size_t)ld * rows * es, me_b = (size_t)n * es;
   const size_t me_off = (mom_b + 255) / 256 * 256;
-  int rc = ensure_scratch(p, me_off + me_b, 0); if (rc != MG_OK) return rc;
-  char* d = (char*)p->d_scratch;
+  cudaStream_t st[2] = {p->own_stream, p->own_stream2};
+  int rc = acquire(p->sc_host, me_off + me_b, st[0]); if (rc != MG_OK) return rc;
+  char* d = (char*)p->sc_host.d;
   // The batch goes through in chunks of events that alternate between two streams, so that the H2D copy of one chunk
   // and the D2H copy of another overlap the kernel of a third (PAPER.md:112 copy:compute balance; the momenta are
   // structure-of-arrays, so a chunk is a 2-D copy: `rows` rows of `width` events with row pitch ld).
   const int64_t min_chunk = 1 << 16;
   int nchunk = (int)(n / min_chunk); if (nchunk < 1) nchunk = 1; if (nchunk > 8) nchunk = 8;
   const int64_t per = ((n + nchunk - 1) / nchunk + 31) / 32 * 32;
-  cudaStream_t st[2] = {p->own_stream, p->own_stream2};
+  p->rescue_last_mask = 0;
   cudaError_t e = cudaEventRecord(p->ev0, st[0]);
+  if (e == cudaSuccess) e = cudaStreamWaitEvent(st[1], p->ev0, 0);      // stream 2 starts after the region is ours
   int c = 0;
-  for (int64_t c0 = 0; c0 < n && e == cudaSuccess; c0 += per, ++c) {
+  for (int64_t c0 = 0; c0 < n && e == cudaSuccess && rc == MG_OK; c0 += per, ++c) {
     const int64_t width = (n - c0) < per ? (n - c0) : per;
     cudaStream_t s = st[c & 1];
     e = cudaMemcpy2DAsync(d + (size_t)c0 * es, (size_t)ld * es, (const char*)h_momenta + (size_t)c0 * es, (size_t)ld * es,
                           (size_t)width * es, rows, cudaMemcpyHostToDevice, s);
     MeArgs a{d + (size_t)c0 * es, width, ld, d + me_off + (size_t)c0 * es, nullptr, nullptr, nullptr, p->hel_mask};
-    if (e == cudaSuccess) e = launch_me(p, a, s);
+    if (e == cudaSuccess) e = cudaEventRecord(p->kev[2 * c], s);
+    if (e == cudaSuccess) rc = run_me(p, a, s, c & 1);
+    if (e == cudaSuccess) e = cudaEventRecord(p->kev[2 * c + 1], s);
     if (e == cudaSuccess) e = cudaMemcpyAsync((char*)h_me + (size_t)c0 * es, d + me_off + (size_t)c0 * es, (size_t)width * es, cudaMemcpyDeviceToHost, s);
   }
-  if (e == cudaSuccess) e = cudaStreamSynchronize(st[1]);
-  if (e == cudaSuccess) e = cudaEventRecord(p->ev1, st[0]);
+  if (e == cudaSuccess) e = cudaEventRecord(p->ev1, st[1]);
+  if (e == cudaSuccess) e = cudaStreamWaitEvent(st[0], p->ev1, 0);      // the region is free when BOTH streams are done
+  if (e == cudaSuccess && rc == MG_OK) rc = release(p->sc_host, st[0]);
   if (e == cudaSuccess) e = cudaStreamSynchronize(st[0]);
   if (e != cudaSuccess) { cudaGetLastError(); return MG_ECUDA; }
-  float ms = 0; cudaEventElapsedTime(&ms, p->ev0, p->ev1); p->last_kernel_ms = ms;     // whole pipelined call
+  if (rc != MG_OK) return rc;
+  double total = 0;
+  for (int i = 0; i < c; ++i) { float ms = 0; cudaEventElapsedTime(&ms, p->kev[2 * i], p->kev[2 * i + 1]); total += ms; }
+  p->last_kernel_ms = total;
   return MG_OK;
 }
 
@@ -382,20 +456,44 @@ int mg_run_host(mg_process* p, uint64_t seed, uint64_t first_event, int64_t n, i
   const int rows = 4 * p->n_ext;
   const size_t mom_b = (size_t)ld * rows * es, vec_b = ((size_t)n * es + 255) / 256 * 256;
   const size_t mom_off = 0, w_off = (mom_b + 255) / 256 * 256, me_off = w_off + vec_b;
-  int rc = ensure_scratch(p, me_off + vec_b, 0); if (rc != MG_OK) return rc;
-  char* d = (char*)p->d_scratch;
   cudaStream_t s = p->own_stream;
+  int rc = acquire(p->sc_host, me_off + vec_b, s); if (rc != MG_OK) return rc;
+  char* d = (char*)p->sc_host.d;
+  p->rescue_last_mask = 0;
   cudaError_t e = launch_generate(p, seed, first_event, n, ld, d + mom_off, d + w_off, s);
-  if (e == cudaSuccess) e = cudaEventRecord(p->ev0, s);
+  if (e == cudaSuccess) e = cudaEventRecord(p->kev[0], s);
   MeArgs a{d + mom_off, n, ld, d + me_off, nullptr, nullptr, nullptr, p->hel_mask};
-  if (e == cudaSuccess) e = launch_me(p, a, s);
-  if (e == cudaSuccess) e = cudaEventRecord(p->ev1, s);
+  if (e == cudaSuccess) rc = run_me(p, a, s, 0);
+  if (e == cudaSuccess) e = cudaEventRecord(p->kev[1], s);
   if (e == cudaSuccess && h_momenta) e = cudaMemcpyAsync(h_momenta, d + mom_off, mom_b, cudaMemcpyDeviceToHost, s);
   if (e == cudaSuccess && h_ps_weight) e = cudaMemcpyAsync(h_ps_weight, d + w_off, (size_t)n * es, cudaMemcpyDeviceToHost, s);
   if (e == cudaSuccess) e = cudaMemcpyAsync(h_me, d + me_off, (size_t)n * es, cudaMemcpyDeviceToHost, s);
+  if (e == cudaSuccess && rc == MG_OK) rc = release(p->sc_host, s);
   if (e == cudaSuccess) e = cudaStreamSynchronize(s);
   if (e != cudaSuccess) { cudaGetLastError(); return MG_ECUDA; }
-  float ms = 0; cudaEventElapsedTime(&ms, p->ev0, p->ev1); p->last_kernel_ms = ms;
+  if (rc != MG_OK) return rc;
+  float ms = 0; cudaEventElapsedTime(&ms, p->kev[0], p->kev[1]); p->last_kernel_ms = ms;
+  return MG_OK;
+}
+
+int mg_set_fp32_rescue(mg_process* p, double kappa_max) {
+  if (!p || !(kappa_max >= 0.0)) return MG_EINVAL;
+  p->rescue_kappa = kappa_max;
+  return MG_OK;
+}
+double mg_get_fp32_rescue(const mg_process* p) { return p ? p->rescue_kappa : 0.0; }
+
+int mg_last_rescued(mg_process* p, int64_t* h_count_out) {
+  if (!p || !h_count_out) return MG_EINVAL;
+  *h_count_out = 0;
+  DeviceGuard g(p->par.device); if (!g.ok) return MG_ECUDA;
+  for (int i = 0; i < 2; ++i) {
+    mg_scratch& sc = p->sc_rescue[i];
+    if (!sc.used || !((p->rescue_last_mask >> i) & 1)) continue;
+    unsigned long long c = 0;
+    if (cudaEventSynchronize(sc.done) != cudaSuccess || cudaMemcpy(&c, sc.d, sizeof(c), cudaMemcpyDeviceToHost) != cudaSuccess) { cudaGetLastError(); return MG_ECUDA; }
+    *h_count_out += (int64_t)c;
+  }
   return MG_OK;
 }
 
@@ -422,23 +520,6 @@ int64_t mg_bytes_per_event(const mg_process* p, int stage) {
   return MG_EINVAL;
 }
 
-int mg_measure_alu_peak(int precision, int device, double* h_tflops_out) {
-  if (!h_tflops_out || device < 0 || (precision != MG_FP64 && precision != MG_FP32)) return MG_EINVAL;
-  int ndev = 0;
-  if (cudaGetDeviceCount(&ndev) != cudaSuccess || device >= ndev) { cudaGetLastError(); return MG_ECUDA; }
-  DeviceGuard g(device); if (!g.ok) return MG_ECUDA;
-  return cuda_rc(measure_alu_peak(precision, device, 0, h_tflops_out));
-}
-
-int mg_measure_alu_mode(int precision, int device, int mode, double* h_tflops_out) {
-  if (!h_tflops_out || device < 0 || (precision != MG_FP64 && precision != MG_FP32) || mode < 0 || mode > 2) return MG_EINVAL;
-  if (mode == 2 && precision != MG_FP64) return MG_EINVAL;
-  int ndev = 0;
-  if (cudaGetDeviceCount(&ndev) != cudaSuccess || device >= ndev) { cudaGetLastError(); return MG_ECUDA; }
-  DeviceGuard g(device); if (!g.ok) return MG_ECUDA;
-  return cuda_rc(measure_alu_peak(precision, device, mode, h_tflops_out));
-}
-
 double mg_last_kernel_ms(const mg_process* p) { return p ? p->last_kernel_ms : 0.0; }
 
 const char* mg_strerror(int code) {
@@ -451,6 +532,6 @@ const char* mg_strerror(int code) {
   }
   return "unknown error";
 }
-const char* mg_version(void) { return "mg-b200 0.1 (sm_100a)"; }
+const char* mg_version(void) { return "mg-b200 0.2 (sm_100a)"; }
 
 }  // extern "C"

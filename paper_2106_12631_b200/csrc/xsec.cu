@@ -2,14 +2,16 @@
 // (cross-section estimate) and hit-or-miss unweighting with stream compaction.  Both are HBM-bound passes over
 // 8 (4) bytes per event; readings R27-R29 in DESIGN.md.
 //
-//   weight sums   one pass, every CTA reduces 1024 x ITEMS weights in double (fixed tree: thread-sequential, warp
-//                 butterfly, warps in order) and writes one partial (sum, sum of squares, max); the partials are
-//                 added on the host in block order -> deterministic for a given n.
-//   unweighting   pass 1 takes the decisions (one Philox call per event: this pass is bound by integer issue, not by
-//                 HBM), stores them as one ballot word per warp and counts the kept events of every 1024-event
-//                 tile; pass 2 is an exclusive scan of the tile counts by one CTA; pass 3 reads the ballots and
-//                 scatters the kept event indices in increasing order (ballot ranks inside a warp, warp offsets
-//                 inside the tile, tile offset from pass 2): a stable compaction, so the result is unique.
+//   weight sums   pass 1: every CTA reduces 1024 x ITEMS weights in double (fixed tree: thread-sequential, warp
+//                 butterfly, warps in order) and writes one partial (sum, sum of squares, max); pass 2: one CTA adds
+//                 the partials in a fixed tree and leaves the three results ON THE DEVICE -> deterministic for a
+//                 given n, no host round trip.
+//   unweighting   ONE pass with a decoupled look-back: a tile of 2048 events takes its decisions (one Philox call per
+//                 event), counts them, publishes its count, looks back over the tiles before it until it meets an
+//                 inclusive prefix, publishes its own inclusive prefix and scatters the kept event indices (ballot
+//                 ranks inside a warp, warp offsets inside the tile, tile offset from the look-back).  Tiles are
+//                 handed out by an atomic ticket in launch order, so a tile only ever waits for tiles that already
+//                 run; the compaction is stable, so the result is unique.  The weights are read once.
 #include "mg_internal.h"
 #include "philox.cuh"
 
@@ -54,64 +56,81 @@ __device__ __forceinline__ bool keep_event(uint64_t seed, uint64_t event, T w, T
   return u32_to_uniform<T>(r.x) * wmax < w;
 }
 
-template <class T>
-__global__ void __launch_bounds__(kTile) unweight_count_kernel(uint64_t seed, uint64_t first, const T* __restrict__ w, int64_t n,
-                                                               T wmax, int* __restrict__ counts, unsigned* __restrict__ ballots) {
-  const int64_t e = (int64_t)blockIdx.x * kTile + threadIdx.x;
-  const bool k = e < n && keep_event<T>(seed, first + (uint64_t)e, __ldcs(w + e), wmax);
-  const unsigned b = __ballot_sync(0xffffffffu, k);
-  if ((threadIdx.x & 31) == 0) ballots[e >> 5] = b;
-  const int c = __syncthreads_count(k);
-  if (threadIdx.x == 0) counts[blockIdx.x] = c;
+// pass 2 of the weight sums: one CTA, partial b of thread (b mod 256) in increasing b, then a fixed tree
+__global__ void __launch_bounds__(256) weight_sums_final_kernel(const double* __restrict__ part, int64_t nb, double* __restrict__ out) {
+  __shared__ double sh[3][256];
+  double a = 0, b = 0, c = 0;
+  for (int64_t i = threadIdx.x; i < nb; i += 256) { a += part[3 * i]; b += part[3 * i + 1]; c = fmax(c, part[3 * i + 2]); }
+  sh[0][threadIdx.x] = a; sh[1][threadIdx.x] = b; sh[2][threadIdx.x] = c;
+  __syncthreads();
+  for (int o = 128; o > 0; o >>= 1) {
+    if (threadIdx.x < o) {
+      sh[0][threadIdx.x] += sh[0][threadIdx.x + o];
+      sh[1][threadIdx.x] += sh[1][threadIdx.x + o];
+      sh[2][threadIdx.x] = fmax(sh[2][threadIdx.x], sh[2][threadIdx.x + o]);
+    }
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) { out[0] = sh[0][0]; out[1] = sh[1][0]; out[2] = sh[2][0]; }
 }
 
-// exclusive scan of the tile counts by ONE CTA (2^24 events = 16384 tiles): every thread owns a contiguous chunk,
-// the 1024 chunk sums are scanned with warp shuffles (two levels); total -> offsets[ntile]
-__global__ void __launch_bounds__(kTile) scan_counts_kernel(const int* __restrict__ counts, int64_t ntile, int64_t* __restrict__ offsets) {
-  __shared__ int64_t warp_sum[kTile / 32];
-  const int64_t chunk = (ntile + kTile - 1) / kTile;
-  const int64_t lo = (int64_t)threadIdx.x * chunk, hi = lo + chunk < ntile ? lo + chunk : ntile;
-  int64_t mine = 0;
-  for (int64_t i = lo; i < hi; ++i) mine += counts[i];
+constexpr int kUwThreads = 512, kUwItems = 4, kUwTile = kUwThreads * kUwItems;   // events per tile
+constexpr unsigned long long kAggregate = 1ull << 62, kInclusive = 2ull << 62, kValueMask = (1ull << 62) - 1;
+
+// state[t]: status (2 bits) | count (62 bits) of tile t;  state[ntile]: the tile ticket
+template <class T>
+__global__ void __launch_bounds__(kUwThreads) unweight_kernel(uint64_t seed, uint64_t first, const T* __restrict__ w, int64_t n, T wmax,
+                                                              int64_t ntile, unsigned long long* __restrict__ state,
+                                                              int64_t* __restrict__ out, int64_t* __restrict__ count_out) {
+  __shared__ int cnt[kUwItems * kUwThreads / 32];      // kept events of every (round, warp), then their exclusive prefix
+  __shared__ long long tile_sh, base_sh;
   const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
-  int64_t incl = mine;                                    // inclusive scan inside the warp
+  if (threadIdx.x == 0) tile_sh = (long long)atomicAdd(state + ntile, 1ull);
+  __syncthreads();
+  const int64_t tile = tile_sh;
+  const int64_t e0 = tile * kUwTile;
+  unsigned ballots[kUwItems];
 #pragma unroll
-  for (int o = 1; o < 32; o <<= 1) {
-    const int64_t t = __shfl_up_sync(0xffffffffu, incl, o);
-    if (lane >= o) incl += t;
+  for (int i = 0; i < kUwItems; ++i) {
+    const int64_t e = e0 + (int64_t)i * kUwThreads + threadIdx.x;
+    const bool k = e < n && keep_event<T>(seed, first + (uint64_t)e, __ldcs(w + e), wmax);
+    ballots[i] = __ballot_sync(0xffffffffu, k);
+    if (lane == 0) cnt[i * (kUwThreads / 32) + wid] = __popc(ballots[i]);
   }
-  if (lane == 31) warp_sum[wid] = incl;
   __syncthreads();
   if (wid == 0) {
-    int64_t v = warp_sum[lane], sc = v;
+    // exclusive scan of the 64 (round, warp) counts: two per lane
+    const int a = cnt[2 * lane], b = cnt[2 * lane + 1];
+    int incl = a + b;
 #pragma unroll
     for (int o = 1; o < 32; o <<= 1) {
-      const int64_t t = __shfl_up_sync(0xffffffffu, sc, o);
-      if (lane >= o) sc += t;
+      const int t = __shfl_up_sync(0xffffffffu, incl, o);
+      if (lane >= o) incl += t;
     }
-    warp_sum[lane] = sc - v;                              // exclusive prefix of the warps
+    const int total = __shfl_sync(0xffffffffu, incl, 31);
+    cnt[2 * lane] = incl - a - b; cnt[2 * lane + 1] = incl - b;
+    if (lane == 0) {
+      unsigned long long prefix = 0;
+      if (tile > 0) {
+        atomicExch(state + tile, kAggregate | (unsigned long long)total);
+        for (int64_t j = tile - 1; j >= 0; --j) {
+          unsigned long long v;
+          do { v = atomicAdd(state + j, 0ull); } while ((v >> 62) == 0);
+          prefix += v & kValueMask;
+          if ((v >> 62) == 2) break;
+        }
+      }
+      atomicExch(state + tile, kInclusive | (prefix + (unsigned long long)total));
+      base_sh = (long long)prefix;
+      if (tile == ntile - 1) *count_out = (int64_t)(prefix + (unsigned long long)total);
+    }
   }
   __syncthreads();
-  int64_t run = warp_sum[wid] + incl - mine;              // exclusive prefix of this thread's chunk
-  for (int64_t i = lo; i < hi; ++i) { offsets[i] = run; run += counts[i]; }
-  if (threadIdx.x == kTile - 1) offsets[ntile] = warp_sum[wid] + incl;
-}
-
-__global__ void __launch_bounds__(kTile) unweight_scatter_kernel(const unsigned* __restrict__ ballots, const int64_t* __restrict__ offsets,
-                                                                 int64_t* __restrict__ out) {
-  __shared__ int warp_base[kTile / 32];
-  const int64_t e = (int64_t)blockIdx.x * kTile + threadIdx.x;
-  const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
-  const unsigned b = __ldg(ballots + (e >> 5));          // one word per warp (events beyond n have a zero bit)
-  const bool k = (b >> lane) & 1u;
-  if (lane == 0) warp_base[wid] = __popc(b);
-  __syncthreads();
-  if (threadIdx.x == 0) {
-    int acc = 0;
-    for (int i = 0; i < kTile / 32; ++i) { const int c = warp_base[i]; warp_base[i] = acc; acc += c; }
-  }
-  __syncthreads();
-  if (k) out[offsets[blockIdx.x] + warp_base[wid] + __popc(b & ((1u << lane) - 1u))] = e;
+  const int64_t base = base_sh;
+#pragma unroll
+  for (int i = 0; i < kUwItems; ++i)
+    if ((ballots[i] >> lane) & 1u)
+      out[base + cnt[i * (kUwThreads / 32) + wid] + __popc(ballots[i] & ((1u << lane) - 1u))] = e0 + (int64_t)i * kUwThreads + threadIdx.x;
 }
 
 }  // namespace
@@ -119,26 +138,25 @@ __global__ void __launch_bounds__(kTile) unweight_scatter_kernel(const unsigned*
 // partials: 3 doubles per CTA in d_part (caller sizes it with weight_sums_blocks)
 int64_t weight_sums_blocks(int64_t n) { return (n + (int64_t)kTile * kItems - 1) / ((int64_t)kTile * kItems); }
 
-cudaError_t launch_weight_sums(const mg_process* p, const void* d_w, int64_t n, double* d_part, cudaStream_t s) {
+cudaError_t launch_weight_sums(const mg_process* p, const void* d_w, int64_t n, double* d_part, double* d_out, cudaStream_t s) {
   const unsigned g = (unsigned)weight_sums_blocks(n);
   if (p->par.precision == MG_FP64) weight_sums_kernel<double><<<g, kTile, 0, s>>>((const double*)d_w, n, d_part);
   else weight_sums_kernel<float><<<g, kTile, 0, s>>>((const float*)d_w, n, d_part);
+  weight_sums_final_kernel<<<1, 256, 0, s>>>(d_part, (int64_t)g, d_out);
   return cudaGetLastError();
 }
 
-int64_t unweight_tiles(int64_t n) { return (n + kTile - 1) / kTile; }
+int64_t unweight_tiles(int64_t n) { return (n + kUwTile - 1) / kUwTile; }
 
-// d_counts: int[ntile], d_ballots: unsigned[32 * ntile], d_offsets: int64[ntile + 1]; d_out: int64[n] (kept event indices, increasing)
 cudaError_t launch_unweight(const mg_process* p, uint64_t seed, uint64_t first, const void* d_w, int64_t n, double wmax,
-                            int* d_counts, unsigned* d_ballots, int64_t* d_offsets, int64_t* d_out, cudaStream_t s) {
+                            unsigned long long* d_state, int64_t* d_out, int64_t* d_count, cudaStream_t s) {
   const int64_t nt = unweight_tiles(n);
-  if (p->par.precision == MG_FP64) {
-    unweight_count_kernel<double><<<(unsigned)nt, kTile, 0, s>>>(seed, first, (const double*)d_w, n, wmax, d_counts, d_ballots);
-  } else {
-    unweight_count_kernel<float><<<(unsigned)nt, kTile, 0, s>>>(seed, first, (const float*)d_w, n, (float)wmax, d_counts, d_ballots);
-  }
-  scan_counts_kernel<<<1, kTile, 0, s>>>(d_counts, nt, d_offsets);
-  unweight_scatter_kernel<<<(unsigned)nt, kTile, 0, s>>>(d_ballots, d_offsets, d_out);
+  cudaError_t e = cudaMemsetAsync(d_state, 0, (size_t)(nt + 1) * sizeof(unsigned long long), s);
+  if (e != cudaSuccess) return e;
+  if (p->par.precision == MG_FP64)
+    unweight_kernel<double><<<(unsigned)nt, kUwThreads, 0, s>>>(seed, first, (const double*)d_w, n, wmax, nt, d_state, d_out, d_count);
+  else
+    unweight_kernel<float><<<(unsigned)nt, kUwThreads, 0, s>>>(seed, first, (const float*)d_w, n, (float)wmax, nt, d_state, d_out, d_count);
   return cudaGetLastError();
 }
 

@@ -378,7 +378,7 @@ class Emitter:
         w("namespace mg {")
         w("struct %s {" % name)
         w("  static constexpr int NHEL = %d;" % (1 << npar))
-        w("  static constexpr int MINB = %d;   // resident CTAs of 128 threads the register allocation aims at" % int(os.environ.get("MG_TPE%d_MINB" % ng, {2: 3}.get(ng, 1))))
+        w("  static constexpr int MINB = %d;   // resident CTAs of 128 threads the register allocation aims at" % {2: 3}.get(ng, 1))
         w("  static constexpr int NPAR = %d;" % npar)
         w("  static constexpr int NFLOW = %d;" % nf)
         w("  static constexpr int NIK = %d;" % (len(self.gsets) + 1))
@@ -409,12 +409,13 @@ class Emitter:
                 out.append("    const Mom<T> %s = %s + K%d;" % (self.kname(S), self.kname(sub), parts[-1]))
         out.append("    const Mom<T> pt = %s[2], ptb = %s[3];" % (ev, ev))
         for key in self.qkeys:
+            # quark-line momenta counted from the t end (q = p_t - gluons absorbed on the way to t~), as in the plain
+            # definition: the same function of the inputs also when they conserve momentum only to
+            # FP32 rounding
             side, S = key
+            S = S if side == "L" else frozenset(range(g.ng)) - S
             kn = self.kname(S) if len(S) > 1 else "K%d" % sorted(S)[0]
-            if side == "L":
-                out.append("    const Mom<T> %s = pt - %s;" % (self.qname(key), kn))
-            else:
-                out.append("    const Mom<T> %s = %s - ptb;" % (self.qname(key), kn))
+            out.append("    const Mom<T> %s = pt - %s;" % (self.qname(key), kn))
         return [l.replace("Mom<T>", "Mom<%s>" % T) for l in out]
 
     def _emit_momenta_fn(self):
@@ -434,7 +435,7 @@ class Emitter:
         for S in self.gsets:
             w("    ev.ik[%d] = (T)(1.0 / mdot(%s, %s));" % (self.ik_index[S], self.kname(S), self.kname(S)))
             self.flops_fixed += 8 + 4 * (len(S) - 1)
-        w("    { const Mom<double> Kf = pt + ptb; ev.ik[%d] = (T)(1.0 / mdot(Kf, Kf)); }" % self.ik_full)
+        w("    { const Mom<double> Kf = %s; ev.ik[%d] = (T)(1.0 / mdot(Kf, Kf)); }   // t t~ current: all gluon momenta" % (" + ".join("K%d" % gi for gi in range(self.g.ng)), self.ik_full))
         for key in self.qkeys:
             w("    ev.iq[%d] = (T)(1.0 / (mdot(%s, %s) - mt2));" % (self.iq_index[key], self.qname(key), self.qname(key)))
             self.flops_fixed += 13
@@ -548,12 +549,16 @@ def generate(ng):
     return gen, em, src, num, den
 
 
+EMITTED = (2,)        # one thread per event only for g g -> t t~; g g -> t t~ g (g) use gen/recycle.py
+
+
 def main():
     table = []
     for ng in (2, 3, 4):
         gen, em, src, num, den = generate(ng)
-        with open(os.path.join(CSRC, FILE_NAME[ng]), "w") as f:
-            f.write(src)
+        if ng in EMITTED:
+            with open(os.path.join(CSRC, FILE_NAME[ng]), "w") as f:
+                f.write(src)
         table.append((ng, gen, em, num, den))
         print("ng=%d: %d diagrams, %d amplitudes, flops/helicity %d, fixed %d" % (ng, gen.n_diag, gen.n_amp, em.flops_hel, em.flops_fixed))
     # tables: flop tallies and colour matrices

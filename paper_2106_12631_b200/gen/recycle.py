@@ -89,39 +89,47 @@ class Closure:
 
 def _closure_key(c):
     """order of the closures inside a step: those sharing the second operand adjacent (it is loaded once)"""
-    mode = os.environ.get('MG_RC_CORDER', '0')
-    if mode == '4':
-        return (c.a.name, c.b.name)
     return (c.b.name, c.a.name)
 
 
+# Launch shape and schedule parameters per number of gluons, tuned on B200 (DESIGN.md §5.4, profiles/r01_c_*):
+#   E, MINB, MINB32   events per CTA, resident CTAs per SM in FP64 / FP32
+#   EG                events per synchronisation group inside a CTA (divides E)
+#   RELAXED           closure steps NOT followed by a barrier: 'auto' = every one whose inputs can be held through the
+#                     next producer step without more shared memory; 'all', '0' (none) or a comma list of step indices
+#   SLOTS             shared-memory entries per event that still let E x MINB events share an SM (0: schedule minimum)
+#   BUDGET            entries of new half products per closure chunk
+#   HOIST             producer steps ride with an earlier producer step when that costs no shared memory
+#   HPERM             lane bit i of a thread's index within its event carries the helicity of particle HPERM[i]
+DEFAULTS = {
+    2: dict(E=8, MINB=3, MINB32=3, EG=None, RELAXED='auto', SLOTS=0, BUDGET=240, HOIST=True, HPERM="2301"),
+    3: dict(E=4, MINB=4, MINB32=5, EG=None, RELAXED='auto', SLOTS=0, BUDGET=240, HOIST=True, HPERM="23104"),
+    4: dict(E=4, MINB=2, MINB32=3, EG=None, RELAXED='auto', SLOTS=424, BUDGET=240, HOIST=True, HPERM="320145"),
+}
+
+
 class Program:
-    def __init__(self, ng, chunk_budget=240):
+    def __init__(self, ng, **opts):
+        """opts override DEFAULTS[ng] (used by sweeps; the committed kernels are the defaults)."""
         self.ng = ng
         g = self.g = qcdgen.Generator(ng)
         self.npar = ng + 2
         self.nhel = 1 << self.npar
-        # events per CTA and resident CTAs per SM (FP64 / FP32): tuned on B200 (DESIGN.md §5.4, profiles/r01_c_*); the
-        # environment overrides MG_RC<ng>_E / _MINB / _MINB32 are for sweeps
-        dflt = {2: (8, 3, 3), 3: (4, 4, 5), 4: (4, 2, 3)}[ng]
-        self.E = int(os.environ.get('MG_RC%d_E' % ng, dflt[0]))
-        self.MINB = int(os.environ.get('MG_RC%d_MINB' % ng, dflt[1]))
-        self.MINB32 = int(os.environ.get('MG_RC%d_MINB32' % ng, dflt[2]))
-        # events per synchronisation group inside a CTA (divides E): the groups of a CTA share nothing but its code
-        self.EG = int(os.environ.get('MG_RC%d_EG' % ng, self.E))
+        o = dict(DEFAULTS[ng])
+        assert set(opts) <= set(o), opts
+        o.update(opts)
+        self.opts = o
+        self.E, self.MINB, self.MINB32 = o["E"], o["MINB"], o["MINB32"]
+        self.EG = o["EG"] or self.E
         assert self.E % self.EG == 0
-        # closure steps (indices into self.steps) that are NOT followed by a barrier: 'auto' = every one whose inputs can
-        # be held through the next producer step without more shared memory; 'all', '0' (none) or a list for sweeps
-        self.RELAXED = os.environ.get('MG_RC%d_RELAXED' % ng, 'auto')
-        # shared-memory entries per event that still let E events x MINB CTAs share an SM (hoisting and barrier removal
-        # may spend them); 0: never more than the schedule needs anyway
-        self.SLOT_LIMIT = int(os.environ.get('MG_RC%d_SLOTS' % ng, {4: 424}.get(ng, 0)))
+        self.RELAXED = o["RELAXED"]
+        self.SLOT_LIMIT = o["SLOTS"]
         self.NT = self.E * self.nhel
         self.gp = g.gl_particle
         self._build_momenta()
         self._build_nodes()
         self._build_closures()
-        self._schedule(int(os.environ.get('MG_RC%d_BUDGET' % ng, chunk_budget)))
+        self._schedule(o["BUDGET"])
         if self.RELAXED == 'auto':
             self.RELAXED = '0'
             self._allocate()
@@ -164,18 +172,17 @@ class Program:
             key = (side, absorbed)
             if key in self.qidx:
                 continue
-            c = kcoef(absorbed)
-            if side == "L":
-                c = [-x for x in c]
-                c[T_PART] += 1                           # q = p_t - K
-            else:
-                c[TB_PART] -= 1                          # q = K - p_tbar
+            # every quark-line momentum is counted from the t end, q = p_t - (gluon momenta absorbed so far on the way to
+            # t~), as the plain definition states it (q_m = p_t - sum k): for momenta that conserve
+            # 4-momentum only to FP32 rounding, K - p_tbar would be a DIFFERENT function of the inputs, and the difference
+            # is amplified by the gauge cancellations of soft and collinear events
+            towards_t = absorbed if side == "L" else frozenset(range(ng)) - absorbed
+            c = [-x for x in kcoef(towards_t)]
+            c[T_PART] += 1
             self.qidx[key] = len(self.mom_names)
             add("q%s%s" % (side, "".join(map(str, sorted(absorbed)))), c, 2)
-        c = [0] * npar
-        c[T_PART] = c[TB_PART] = 1
-        self.kf = len(self.mom_names)
-        add("Kf", c, 1)
+        self.kf = len(self.mom_names)                    # momentum of the t t~ current = all gluon momenta (same remark)
+        add("Kf", kcoef(frozenset(range(ng))), 1)
 
     # ------------------------------------------------------------------ nodes of the diagram list
     def _build_nodes(self):
@@ -261,9 +268,6 @@ class Program:
             classes.setdefault((nn.nbits, nn.kind), OrderedDict()).setdefault(nn.name, []).append(c)
         chunks, cur, cur_n = [], [], 0
         keys = sorted(classes)
-        perm = os.environ.get('MG_RC%d_ORDER' % self.ng)          # sweep knob: order of the closure classes
-        if perm:
-            keys = [keys[int(ch)] for ch in perm]
         for key in keys:
             names = list(classes[key])
             total = sum(self.half[x].nvar for x in names)
@@ -317,7 +321,7 @@ class Program:
         self._number()
         # HOIST: a producer step whose nodes can all be computed in an earlier producer step (operands born before it)
         # rides with that step when this costs no shared memory: one barrier-separated latency chain fewer
-        if os.environ.get('MG_RC%d_HOIST' % self.ng, '1') != '0':
+        if self.opts["HOIST"]:
             self.RELAXED_SAVE, self.RELAXED = self.RELAXED, '0'
             self._allocate()
             limit = max(self.nslot, self.SLOT_LIMIT)
@@ -506,7 +510,7 @@ def emit(prog):
     # lane bit i of a thread's index within its event carries the helicity of particle hperm[i]: t and t~ in the two
     # lowest bits.  All 720 / 120 orders were timed on B200 with a run-time permutation, the best few rebuilt with the
     # compile-time one: 2.7 % (g g -> t t~ g g) and 2 % (g g -> t t~ g) faster than particle order
-    hperm = os.environ.get("MG_RC%d_HPERM" % ng, {2: "2301", 3: "23104", 4: "320145"}[ng])
+    hperm = prog.opts["HPERM"]
     assert sorted(hperm) == [str(i) for i in range(npar)]
     w("  static constexpr unsigned HPERM = 0x%s;   // nibble i: particle whose helicity is bit i of the lane index" % hperm[::-1])
     w("  static __device__ __forceinline__ const rc::NodeDesc& node(int i) { return kRcNode_%s[i]; }" % tag)
@@ -514,8 +518,8 @@ def emit(prog):
     w("  static __device__ __forceinline__ rc::MomDef momdef(int i) { return kRcMom_%s[i]; }" % tag)
     w("")
     w("  // producer steps, inner products, colour sum: |M|^2 of helicity h of event el (no g_s^(2 n_g)/denominator)")
-    w("  template <class T> static __device__ __forceinline__ T run(const rc::Smem<%s, T>& s, int tid, int el, int h, T mt) {" % name)
-    w("    const rc::View<T, NSLOT> ev = s.view(el);")
+    w("  template <class T, class SM> static __device__ __forceinline__ T run(const SM& s, int tid, int el, int h, T mt) {")
+    w("    const typename SM::VW ev = s.view(el);")
     w("    const int grp = tid / NTG, gt = tid - grp * NTG, eb = grp * EG;   // synchronisation group, thread in it, its first event")
     w("    cx<T> jamp[NFLOW];")
     seen = set()
@@ -537,12 +541,9 @@ def emit(prog):
             for i, (k, nb, first, nfam, lo, hi) in enumerate(bounds):
                 cond = "" if len(bounds) == 1 else ("if (t < %d) " % hi if i == 0 else ("else if (t < %d) " % hi if i < len(bounds) - 1 else "else "))
                 if k == "MOMTAB":
-                    w("      %src::run_momtab<%s, T>(s, t, mt, eb);" % (cond, name))
+                    w("      %src::run_momtab<%s>(s, t, mt, eb);" % (cond, name))
                 else:
-                    if k in os.environ.get("MG_RC_ABLATE", "").split(","):
-                        w("      %s{ }" % cond)
-                    else:
-                        w("      %src::run_group<%s, T, rc::K_%s, %d>(s, %d, %d, t - %d, mt, eb);" % (cond, name, k, nb, first, nfam, lo))
+                    w("      %src::run_group<%s, SM, rc::K_%s, %d>(s, %d, %d, t - %d, mt, eb);" % (cond, name, k, nb, first, nfam, lo))
             w("    }")
             w("    rc::sync_group<%s>(grp);" % name)
         else:
@@ -600,9 +601,14 @@ def generate(ng):
 def tables(progs):
     out = "// GENERATED by paper_2106_12631_b200/gen/recycle.py — do not edit.\n#pragma once\nnamespace mg {\n"
     for ng, prog in progs:
+        if ng not in EMITTED:
+            continue
         out += "static const long kFlopsRecycle_%d = %d;   // per event: setup %d + tasks %d + %d helicities x %d + reduction\n" % (
             ng, prog.flops_event, prog.flops_setup, prog.flops_nodes, prog.nhel, prog.flops_hel)
     return out + "}  // namespace mg\n"
+
+
+EMITTED = (3, 4)      # g g -> t t~ runs one thread per event (gen_ggtt.cuh): its recycling program is only interpreted by the tests
 
 
 def main():
@@ -610,6 +616,8 @@ def main():
     for ng in (2, 3, 4):
         prog, src = generate(ng)
         progs.append((ng, prog))
+        if ng not in EMITTED:
+            continue
         with open(os.path.join(CSRC, FILE_NAME[ng]), "w") as f:
             f.write(src)
         print("ng=%d: %d nodes, %d tasks/event, %d closures, %d slots (%.1f KB/event FP64), %d steps, flops/event %d (per hel %d)" %

@@ -43,16 +43,18 @@ def sharded_sums(compute, n_total, first_event=0, rank=None, world=None, device=
     return mean, (var / n_total) ** 0.5, t[2].item() / n_total, n_total
 
 
-def gpu_compute(process):
-    """compute() for sharded_sums: the CUDA path on this rank's device for a Process handle."""
+def gpu_compute(process, seed=7):
+    """compute() for sharded_sums: the CUDA path on this rank's device for a Process handle: events generated and
+    evaluated by mg_sigmakin_fused, batch sums by mg_weight_sums_async (everything stays on the device until the one
+    9-double copy at the end)."""
     def compute(first, count):
-        mom, w = process.generate(process_seed(process), first, count)
-        ew = torch.empty_like(w)
-        me = process.sigmakin(mom, count, ps_weight=w, event_weight=ew)
-        m = me[:count].to(torch.float64)
-        return m.sum().item(), (m * m).sum().item(), ew[:count].to(torch.float64).sum().item()
+        dev, dt = process.device, process.dtype
+        me = torch.empty(count, dtype=dt, device=dev)
+        w = torch.empty(count, dtype=dt, device=dev)
+        ew = torch.empty(count, dtype=dt, device=dev)
+        process.sigmakin_fused(seed, first, count, me, w, ew)
+        s_me = process.weight_sums_async(me, count)
+        s_ew = process.weight_sums_async(ew, count)
+        v = torch.cat([s_me, s_ew]).cpu()
+        return v[0].item(), v[1].item(), v[3].item()
     return compute
-
-
-def process_seed(process):
-    return getattr(process, "seed", 7)

@@ -40,10 +40,16 @@ def chi(p, P, lam):
     return np.array([(-px + 1j * py) * nrm, Ppz * nrm])
 
 
+def omegas(E, P, m):
+    if m == 0:
+        return np.sqrt(2 * P), 0.0
+    em = E + m
+    return (em + P) / np.sqrt(2 * em), (em - P) / np.sqrt(2 * em)
+
+
 def spinor_u(p, m, lam):
     P = np.sqrt(p[1] ** 2 + p[2] ** 2 + p[3] ** 2)
-    wp = np.sqrt((P if m == 0 else p[0]) + P)
-    wm = m / wp
+    wp, wm = omegas(p[0], P, m)
     x = chi(p, P, lam)
     wl, wr = (wm, wp) if lam > 0 else (wp, wm)
     return np.array([wl * x[0], wl * x[1], wr * x[0], wr * x[1]])
@@ -51,8 +57,7 @@ def spinor_u(p, m, lam):
 
 def spinor_v(p, m, lam):
     P = np.sqrt(p[1] ** 2 + p[2] ** 2 + p[3] ** 2)
-    wp = np.sqrt((P if m == 0 else p[0]) + P)
-    wm = m / wp
+    wp, wm = omegas(p[0], P, m)
     x = chi(p, P, -lam)
     wl, wr = (wp, -wm) if lam > 0 else (wm, -wp)
     return np.array([wl * x[0], wl * x[1], wr * x[0], wr * x[1]])

@@ -10,7 +10,9 @@ Tolerances (north_star; DESIGN.md "Tolerances"):
          tolerance; the CUDA path evaluates the same map in a form that loses only gamma (rambo.cuh).
          FP32: events with gamma > 32 are held to 1e-5 * gamma/32, counted and printed.
   ME     FP64                     |ME_gpu/ME_oracle - 1| <= 1e-12 per event (oracle fed the GPU's momenta)
-         FP32                     <= 1e-4 per event and <= 1e-6 on the batch mean
+         FP32                     <= 1e-4 per event and <= 1e-6 on the batch mean, every process, unmodified (north_star);
+                                  compared sets of SURVEY.md C10: whole batch for e+e- -> mu+mu- and g g -> t t~, the first
+                                  4096 plus >= 2^16 strided events of the full-size batch for g g -> t t~ g (g)
          ill-conditioned tail (FP64): an event may exceed 1e-12 only if the double oracle itself is more
          than 2.5e-13 away from the long-double oracle on that event; it is then compared with the
          long-double oracle at 1e-10, counted and printed.
@@ -52,6 +54,18 @@ def test_rng_words_bit_exact(mg, process, seed, first, n):
     w = _np(P.rng_words(seed, first, n), n).view(np.uint32)
     ref = oracle.rng_words(seed, first, n, P.n_final)          # [n, nf, 4]
     assert np.array_equal(w, aos_to_soa(ref))
+
+
+@pytest.mark.parametrize("process,seed,n", [(0, 42, 16384), (0, 7, 1 << 24), (1, 7, 1 << 22), (2, 7, 1 << 21), (3, 7, 1 << 20)])
+def test_rng_words_bit_exact_whole_batch(mg, process, seed, n):
+    """the u32 words of one whole BASELINE.json batch per configuration, bit for bit (oracle in chunks)."""
+    P = mg.Process(process)
+    w = P.rng_words(seed, 0, n)
+    chunk = 1 << 20
+    for c0 in range(0, n, chunk):
+        m = min(chunk, n - c0)
+        ref = torch.from_numpy(aos_to_soa(oracle.rng_words(seed, c0, m, P.n_final)).view(np.int32)).to(w.device)
+        assert torch.equal(w[:, c0:c0 + m], ref), (process, c0)
 
 
 @pytest.mark.parametrize("prec", [0, 1])
@@ -185,7 +199,7 @@ def test_me_fp32(mg, process):
     print("me fp32 process %d: n %d, max rel %.2e, mean rel %.2e, nan %d" % (process, n, np.nanmax(rel), mean_rel, np.isnan(me_g).sum()))
     assert np.isfinite(me_g).all()
     assert rel.max() <= 1e-4
-    assert mean_rel <= 1e-6 * (1 if process < 2 else 10)   # P2/P3 small-sample means are dominated by a few events; see DESIGN.md
+    assert mean_rel <= 1e-6
 
 
 @pytest.mark.parametrize("process", PROCS)
@@ -404,15 +418,28 @@ def test_fp32_error_profile(mg, process):
 
 
 # ----------------------------------------------------------------------------- BASELINE.json full sizes
-@pytest.mark.parametrize("process,prec,n,seed,nsample", [
-    (0, 0, 16384, 42, 16384), (0, 0, 1 << 24, 7, 4096), (0, 1, 1 << 24, 7, 4096),
-    (1, 0, 1 << 22, 7, 4096), (1, 1, 1 << 22, 7, 4096), (2, 0, 1 << 21, 7, 1024), (2, 1, 1 << 21, 7, 1024),
-    (3, 0, 1 << 20, 7, 256), (3, 1, 1 << 20, 7, 256)])
-def test_full_size_configs_sampled_parity(mg, process, prec, n, seed, nsample):
+def _compare_set(process, n):
+    """whole batch for e+e- -> mu+mu- and g g -> t t~; the first 4096 events plus 2^16 events strided over
+    the whole index range (ragged positions included) for g g -> t t~ g (g)."""
+    if process < 2:
+        return None
+    idx = np.concatenate([np.arange(min(4096, n)), np.linspace(0, n - 1, 1 << 16).astype(np.int64), [31, 32, n - 2, n - 1]])
+    return np.unique(idx)
+
+
+@pytest.mark.parametrize("process,prec,n,seed", [
+    (0, 0, 16384, 42), (0, 0, 1 << 24, 7), (0, 1, 1 << 24, 7), (1, 0, 1 << 22, 7), (1, 1, 1 << 22, 7),
+    (2, 0, 1 << 21, 7), (2, 1, 1 << 21, 7), (3, 0, 1 << 20, 7), (3, 1, 1 << 20, 7)])
+def test_full_size_configs_parity(mg, process, prec, n, seed):
     """The five configurations of BASELINE.json at their full sizes, in the launch configuration bench.py times
-    (mg_rng -> mg_rambo -> mg_filter_helicities -> mg_sigmakin with the event weight): a strided sample of events
-    covering the whole index range (first, last and ragged positions included) is compared with the oracle fed the
-    GPU's momenta; the whole batch must be finite and positive and its weights must satisfy w = W * ME (R18)."""
+    (mg_rng -> mg_rambo -> mg_filter_helicities -> mg_sigmakin with the event weight), against the oracle fed the GPU's
+    momenta on the compared set of SURVEY.md C10.  north_star's tolerances, unmodified:
+      FP64  <= 1e-12 per event; events above it are counted and must be cases where the double oracle itself is
+            > 2.5e-13 from the long-double oracle (ill-conditioned event), agree with the long-double oracle to 1e-10,
+            and number <= 1e-3 of the compared set (C10: "report the count and the max");
+      FP32  <= 1e-4 per event, <= 1e-6 on the mean of the compared set, no non-finite value.
+    The whole batch must be finite and positive and its weights must satisfy w = W * ME (R18).  The printed lines are
+    the rows of profiles/r02_parity_full_size.md."""
     P = mg.Process(process, prec)
     ld = mg.padded_stride(n)
     rnd = P.rng(seed, 0, n)
@@ -423,18 +450,143 @@ def test_full_size_configs_sampled_parity(mg, process, prec, n, seed, nsample):
     me = P.sigmakin(mom, n, ps_weight=w, event_weight=ew)
     assert bool(torch.isfinite(me[:n]).all().item()) and bool((me[:n] > 0).all().item())
     assert torch.equal(ew[:n], w[:n] * me[:n])
-    idx = np.unique(np.concatenate([np.linspace(0, n - 1, nsample).astype(np.int64), [0, 1, 31, 32, n - 2, n - 1]]))
-    tidx = torch.from_numpy(idx).to(P.device)
-    mom_s = mom[:, tidx].cpu().numpy().astype(np.float64)
-    me_s = me[tidx].cpu().numpy().astype(np.float64)
-    me_o = oracle.me(process, soa_to_aos(mom_s, P.n_external))
-    rel = np.abs(me_s / me_o - 1)
-    print("full size process %d prec %d n %d: %d sampled events, max rel %.2e" % (process, prec, n, len(idx), rel.max()))
-    if prec == 0:
-        bad = rel > 1e-12
-        if bad.any():                     # ill-conditioned tail: decided by the long-double oracle (header of this file)
-            me_l = oracle.me(process, soa_to_aos(mom_s[:, bad], P.n_external), long_double=True)
-            assert (np.abs(me_o[bad] / me_l - 1) > 2.5e-13).all() and (np.abs(me_s[bad] / me_l - 1) < 1e-10).all()
-            assert bad.sum() <= max(1, len(idx) // 1000)
+    idx = _compare_set(process, n)
+    if idx is None:
+        mom_s, me_s = mom[:, :n], me[:n]
     else:
+        tidx = torch.from_numpy(idx).to(P.device)
+        mom_s, me_s = mom[:, tidx], me[tidx]
+    me_s = me_s.cpu().numpy().astype(np.float64)
+    m = me_s.shape[0]
+    me_o = np.empty(m)
+    chunk = 1 << 21
+    for c0 in range(0, m, chunk):                       # the whole-batch sets go through the oracle in chunks
+        c1 = min(m, c0 + chunk)
+        me_o[c0:c1] = oracle.me(process, soa_to_aos(mom_s[:, c0:c1].cpu().numpy().astype(np.float64), P.n_external))
+    rel = np.abs(me_s / me_o - 1)
+    mean_bias = me_s.mean() / me_o.mean() - 1
+    line = "full size: process %d %s n %d compared %d: max rel %.2e  p99.9 %.2e  mean bias %+.2e" % (
+        process, "fp64" if prec == 0 else "fp32", n, m, rel.max(), np.quantile(rel, 0.999), mean_bias)
+    if prec == 0:
+        bad = np.nonzero(rel > 1e-12)[0]
+        line += "  above 1e-12: %d" % len(bad)
+        if len(bad):                      # ill-conditioned tail: decided by the long-double oracle (header of this file)
+            mom_b = mom_s[:, torch.from_numpy(bad).to(P.device)].cpu().numpy()
+            me_l = oracle.me(process, soa_to_aos(mom_b, P.n_external), long_double=True)
+            own, res = np.abs(me_o[bad] / me_l - 1), np.abs(me_s[bad] / me_l - 1)
+            line += " (vs long double: gpu max %.2e, double oracle's own max %.2e)" % (res.max(), own.max())
+            print(line)
+            assert (own > 2.5e-13).all() and (res < 1e-10).all()
+            assert len(bad) <= max(1, m // 1000)
+        else:
+            print(line)
+    else:
+        if process >= 2:
+            line += "  recomputed in double: %d of %d" % (P.last_rescued(), n)
+        print(line)
+        assert np.isfinite(me_s).all()
         assert rel.max() <= 1e-4
+        assert abs(mean_bias) <= 1e-6
+
+
+# ----------------------------------------------------------------------------- mixed precision
+@pytest.mark.parametrize("process", [2, 3])
+def test_fp32_rescue_is_a_function_of_the_event_only(mg, process):
+    """The double-precision pass over the ill-conditioned events of an FP32 batch (mg_set_fp32_rescue): which events it
+    takes depends on their momenta only, so results do not depend on the batch split; switching it off changes only
+    the listed events; the recomputed values are the FP64 kernel's on the same FP32 momenta, rounded to float."""
+    n = 20000 + 13
+    P = mg.Process(process, 1)
+    assert P.fp32_rescue() > 0
+    mom, _ = P.generate(7, 5000, n)
+    me = P.sigmakin(mom, n)[:n].clone()
+    k = P.last_rescued()
+    assert 0 < k < n // 5
+    a = P.sigmakin(mom[:, :8000].contiguous(), 8000)[:8000]
+    b = P.sigmakin(mom[:, 8000:].contiguous(), n - 8000)[:n - 8000]
+    assert torch.equal(torch.cat([a, b]), me)
+    P.set_fp32_rescue(0.0)
+    pure = P.sigmakin(mom, n)[:n].clone()
+    assert P.last_rescued() == 0
+    changed = (pure != me).sum().item()
+    assert 0 < changed <= k
+    P64 = mg.Process(process, 0)
+    me64 = P64.sigmakin(mom.to(torch.float64), n)[:n]
+    diff = pure != me
+    assert torch.equal(me[diff], me64[diff].to(torch.float32))
+    # fused path: same decision from momenta generated in the kernel
+    P.set_fp32_rescue(1000.0)
+    f1 = P.sigmakin_fused(7, 5000, n)
+    k1 = P.last_rescued()
+    mom2, _ = P.generate(7, 5000, n)
+    f2 = P.sigmakin(mom2, n)[:n]
+    assert k1 == P.last_rescued()
+    assert ((f1 / f2) - 1).abs().max().item() <= 2e-5
+
+
+def test_two_streams_share_a_handle_safely(mg):
+    """Scratch regions of a handle are ordered with events (include/mg.h "Streams and threads"): calls that need the
+    same region on two streams give the results of the same calls issued one after the other."""
+    P = mg.Process(3, 1)
+    n = 30000
+    mom_a, _ = P.generate(7, 0, n)
+    mom_b, _ = P.generate(7, 10**6, n)
+    ref_a = P.sigmakin(mom_a, n)[:n].clone()
+    ref_b = P.sigmakin(mom_b, n)[:n].clone()
+    torch.cuda.synchronize()
+    s1, s2 = torch.cuda.Stream(), torch.cuda.Stream()
+    outs = []
+    for rep in range(4):
+        with torch.cuda.stream(s1):
+            xa = P.sigmakin(mom_a, n)
+        with torch.cuda.stream(s2):
+            xb = P.sigmakin(mom_b, n)
+        outs.append((xa, xb))
+    torch.cuda.synchronize()
+    for xa, xb in outs:
+        assert torch.equal(xa[:n], ref_a) and torch.equal(xb[:n], ref_b)
+    # the steps after the path on two streams
+    ew = P.sigmakin_fused(7, 0, n)
+    sums = P.weight_sums(ew, n)
+    with torch.cuda.stream(s1):
+        d1 = P.weight_sums_async(ew, n)
+    with torch.cuda.stream(s2):
+        kept, cnt = P.unweight_async(7, 0, ew, n, sums[2])
+    torch.cuda.synchronize()
+    assert tuple(d1.cpu().tolist()) == sums
+    assert torch.equal(kept[:cnt.item()], P.unweight(7, 0, ew, n, sums[2]))
+
+
+@pytest.mark.parametrize("process,prec,n", [(1, 0, (1 << 17) + 37), (1, 1, 1 << 20), (2, 0, (1 << 17) + 37), (2, 1, (1 << 18) + 5)])
+def test_host_form_chunked_path(mg, process, prec, n):
+    """mg_sigmakin_host with batches of 2^17 events or more: chunks on two streams, 2-D copies of sub-columns with
+    ld > n, ragged last chunk (what bench.py's e2e number times) against mg_sigmakin on the same momenta."""
+    P = mg.Process(process, prec)
+    ld = mg.padded_stride(n) + 64
+    mom = P.empty(4 * P.n_external, n, ld)
+    P.generate(7, 0, n, mom)
+    ref = P.sigmakin(mom, n)[:n].cpu()
+    h_mom = torch.empty((4 * P.n_external, ld), dtype=P.dtype).pin_memory()
+    h_mom.copy_(mom.cpu())
+    h_me = torch.zeros(n, dtype=P.dtype).pin_memory()
+    P.sigmakin_host(h_mom, n, h_me)
+    assert torch.equal(h_me, ref)
+    assert P.last_kernel_ms() > 0
+
+
+def test_sharded_sums_on_one_device(mg):
+    """shard.gpu_compute (the compute leg of the multi-GPU path) on one device: world 1 and two
+    emulated ranks (rank/world passed explicitly) merge to the same sums, which match the oracle on the same events."""
+    from paper_2106_12631_b200 import shard
+    P = mg.Process(2, 0)
+    n = 3000 + 7
+    one = shard.sharded_sums(shard.gpu_compute(P, seed=7), n, first_event=100, rank=0, world=1, device="cuda")
+    parts = []
+    for r in range(2):
+        first, count = shard.event_range(r, 2, n, 100)
+        parts.append(shard.gpu_compute(P, seed=7)(first, count))
+    tot = np.sum(np.array(parts), axis=0)
+    mean = tot[0] / n
+    assert abs(mean / one[0] - 1) < 1e-13 and abs(tot[2] / n / one[2] - 1) < 1e-13
+    me_o, w_o = oracle.pipeline(2, 7, 100, n)
+    assert abs(one[0] / me_o.mean() - 1) < 1e-9 and abs(one[2] / (me_o * w_o).mean() - 1) < 1e-9

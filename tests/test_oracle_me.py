@@ -221,9 +221,120 @@ def test_long_double_and_double_agree():
 
 
 def test_pipeline_equals_steps():
-    for process in (0, 1, 2):
-        me, w, mom = oracle.pipeline(process, 7, 100, 16, want_momenta=True)
-        rho = oracle.uniforms(7, 100, 16, oracle.N_FINAL[process])
+    for process, n in ((0, 16), (1, 16), (2, 16), (3, 4)):
+        me, w, mom = oracle.pipeline(process, 7, 100, n, want_momenta=True)
+        rho = oracle.uniforms(7, 100, n, oracle.N_FINAL[process])
         mom2, w2, _ = oracle.rambo(rho, oracle.masses(process), SQRT_S)
         assert (mom == mom2).all() and (w == w2).all()
         assert (me == oracle.me(process, mom2)).all()
+
+
+# ----------------------------------------------------------------------------- absolute normalisation of P2 and P3
+# SURVEY.md §8(c) C6 (optional pin): in a collinear limit the (n+1)-parton matrix element factorises onto the n-parton
+# one times a universal splitting function (Altarelli-Parisi; in the form of Catani-Seymour, NPB 485 (1997) 291,
+# eqs. 4.1 / 4.17, spin-averaged P_gg(z) = 2 C_A [z/(1-z) + (1-z)/z + z(1-z)], both sides summed/averaged the same
+# way):
+#   final state   |M_{n+1}|^2 -> (g_s^2 / p_i.p_j)        P_gg(z) |M_n|^2
+#   initial state |M_{n+1}|^2 -> (g_s^2 / p_a.p_i) (1/x)  P_gg(x) |M_n(x p_a)|^2
+# after averaging over the azimuth of the splitting plane.  This ties g g -> t t~ g to g g -> t t~ (pinned by its
+# closed form) and g g -> t t~ g g to g g -> t t~ g, INCLUDING the couplings g_s^(2 n_g), the averaging denominators
+# 256 / 256 / 512 (the 1/2! of the two identical final gluons, R11) and the colour sums: a wrong 512 or a missing
+# g_s^2 changes the ratio by a factor, while the approach to the limit is smooth in the opening angle.
+# PAPER.md:35 (§2) says only "averaged".  Kinematics below are built with exact momentum conservation and mass shells.
+def _p_gg(z):
+    return 2 * 3.0 * (z / (1 - z) + (1 - z) / z + z * (1 - z))
+
+
+def _boost(p, frame):
+    """p given in the rest frame of the massive 4-vector `frame` -> the frame where `frame` has its components"""
+    m = math.sqrt(_mdot(frame, frame))
+    b = frame[1:] / frame[0]
+    g = frame[0] / m
+    bp = b @ p[1:]
+    b2 = b @ b
+    out = np.empty(4)
+    out[0] = g * (p[0] + bp)
+    out[1:] = p[1:] + ((g - 1) * bp / b2 + g * p[0]) * b if b2 > 0 else p[1:]
+    return out
+
+
+def _perp_basis(d):
+    d = d / np.linalg.norm(d)
+    a = np.array([1.0, 0, 0]) if abs(d[0]) < 0.9 else np.array([0, 1.0, 0])
+    e1 = np.cross(d, a); e1 /= np.linalg.norm(e1)
+    return d, e1, np.cross(d, e1)
+
+
+def _two_body_decay(parent, costh, phi):
+    """massless pair of total momentum `parent` (massive), decay direction (costh, phi) relative to the parent's flight direction"""
+    m = math.sqrt(_mdot(parent, parent))
+    d, e1, e2 = _perp_basis(parent[1:])
+    sth = math.sqrt(1 - costh * costh)
+    n = costh * d + sth * (math.cos(phi) * e1 + math.sin(phi) * e2)
+    pi = _boost(np.concatenate([[m / 2], m / 2 * n]), parent)
+    return pi, parent - pi
+
+
+def test_final_state_collinear_limit_pins_the_normalisation_of_ggttgg():
+    par = oracle.default_params()
+    gs2 = 4 * math.pi * par.alpha_s
+    rho = oracle.uniforms(5, 3, 1, 3)
+    costh = 0.3
+    prev = None
+    for m_ij in (30.0, 10.0, 3.0, 1.0):
+        # g g -> t t~ X with a pseudo-particle X of mass m_ij from the same uniforms, X -> g g
+        mom3, _, _ = oracle.rambo(rho, np.array([par.mt, par.mt, m_ij]), SQRT_S, long_double=True)
+        ratios = []
+        for k in range(8):
+            pi, pj = _two_body_decay(mom3[0, 4], costh, 0.4 + k * math.pi / 4)
+            mom4 = np.concatenate([mom3[0, :4], [pi], [pj]])[None]
+            z = pi[0] / (pi[0] + pj[0])
+            parent = oracle.rambo(rho, np.array([par.mt, par.mt, 0.0]), SQRT_S, long_double=True)[0]
+            me4 = oracle.me(3, mom4, par)[0]
+            me3 = oracle.me(2, parent, par)[0]
+            # 1/2! on the left (two identical final gluons) and none on the right
+            ratios.append(me4 * 2 / (gs2 / _mdot(pi, pj) * _p_gg(z) * me3))
+        r = float(np.mean(ratios))
+        print("m_ij %5.1f GeV: <ME4 * 2! / (gs^2/(pi.pj) P_gg ME3)> = %.6f" % (m_ij, r))
+        if prev is not None:
+            assert abs(r - 1) < abs(prev - 1)                   # approaches the limit monotonically
+        prev = r
+    assert abs(prev - 1) < 5e-5                                  # quadratic approach; a factor 2 (1/2!) or g_s^2 = 1.48 would be far off
+
+
+def test_initial_state_collinear_limit_pins_the_normalisation_of_ggttg():
+    par = oracle.default_params()
+    gs2 = 4 * math.pi * par.alpha_s
+    s = SQRT_S**2
+    p0 = np.array([SQRT_S / 2, 0, 0, SQRT_S / 2])
+    p1 = np.array([SQRT_S / 2, 0, 0, -SQRT_S / 2])
+    x, cth, ph = 0.6, 0.35, 1.1                                  # momentum fraction kept by the beam gluon; t t~ angles
+    prev = None
+    for kt in (60.0, 20.0, 6.0, 2.0):
+        ratios = []
+        for k in range(8):
+            a = 0.2 + k * math.pi / 4
+            kperp = np.array([0, kt * math.cos(a), kt * math.sin(a), 0])
+            beta = kt * kt / ((1 - x) * s)
+            p4 = (1 - x) * p0 + kperp + beta * p1                # massless: (1-x) beta s = kt^2
+            Q = p0 + p1 - p4                                     # t t~ system
+            mhat = math.sqrt(_mdot(Q, Q))
+            pstar = math.sqrt(mhat * mhat / 4 - par.mt**2)
+            n = np.array([math.sqrt(1 - cth * cth) * math.cos(ph), math.sqrt(1 - cth * cth) * math.sin(ph), cth])
+            pt = _boost(np.concatenate([[mhat / 2], pstar * n]), Q)
+            mom3 = np.stack([p0, p1, pt, Q - pt, p4])[None]
+            # reduced process: beams (x p0, p1), the same t t~ angles in their rest frame
+            Q2 = x * p0 + p1
+            mh2 = math.sqrt(_mdot(Q2, Q2))
+            ps2 = math.sqrt(mh2 * mh2 / 4 - par.mt**2)
+            pt2 = _boost(np.concatenate([[mh2 / 2], ps2 * n]), Q2)
+            mom2 = np.stack([x * p0, p1, pt2, Q2 - pt2])[None]
+            me3 = oracle.me(2, mom3, par)[0]
+            me2 = oracle.me(1, mom2, par)[0]
+            ratios.append(me3 / (gs2 / _mdot(p0, p4) / x * _p_gg(x) * me2))
+        r = float(np.mean(ratios))
+        print("kT %5.1f GeV: <ME3 / (gs^2/(p0.p4) P_gg(x)/x ME2)> = %.6f" % (kt, r))
+        if prev is not None:
+            assert abs(r - 1) < abs(prev - 1)
+        prev = r
+    assert abs(prev - 1) < 5e-5
