@@ -13,9 +13,10 @@ Tolerances (north_star; DESIGN.md "Tolerances"):
          FP32                     <= 1e-4 per event and <= 1e-6 on the batch mean, every process, unmodified (north_star);
                                   compared sets of SURVEY.md C10: whole batch for e+e- -> mu+mu- and g g -> t t~, the first
                                   4096 plus >= 2^16 strided events of the full-size batch for g g -> t t~ g (g)
-         ill-conditioned tail (FP64): an event may exceed 1e-12 only if the double oracle itself is more
-         than 2.5e-13 away from the long-double oracle on that event; it is then compared with the
-         long-double oracle at 1e-10, counted and printed.
+         ill-conditioned tail (FP64, R30): the DOUBLE oracle loses eps/theta^2 in the propagator
+         denominators of collinear pairs (own error up to 2.4e-10 in 2^20 uncut events).  An event above 1e-12
+         against the double oracle is therefore re-compared with the LONG-DOUBLE oracle, where the same 1e-12
+         holds unmodified (the kernels evaluate those denominators in double-double); counted and printed.
 """
 import numpy as np
 import pytest
@@ -185,8 +186,7 @@ def test_me_fp64(mg, process):
         own = np.abs(me_o[bad] / me_l - 1)
         rel_l = np.abs(me_g[bad] / me_l - 1)
         print("   tail vs long double: gpu max %.2e, double oracle's own max %.2e" % (rel_l.max(), own.max()))
-        assert (own > 2.5e-13).all(), "GPU exceeds 1e-12 on a well-conditioned event"
-        assert (rel_l < 1e-10).all()
+        assert (rel_l <= 1e-12).all()
         assert len(bad) <= max(1, n // 1000)
 
 
@@ -434,9 +434,9 @@ def test_full_size_configs_parity(mg, process, prec, n, seed):
     """The five configurations of BASELINE.json at their full sizes, in the launch configuration bench.py times
     (mg_rng -> mg_rambo -> mg_filter_helicities -> mg_sigmakin with the event weight), against the oracle fed the GPU's
     momenta on the compared set of SURVEY.md C10.  north_star's tolerances, unmodified:
-      FP64  <= 1e-12 per event; events above it are counted and must be cases where the double oracle itself is
-            > 2.5e-13 from the long-double oracle (ill-conditioned event), agree with the long-double oracle to 1e-10,
-            and number <= 1e-3 of the compared set (C10: "report the count and the max");
+      FP64  <= 1e-12 per event; events above it against the double oracle are counted, must agree with the
+            long-double oracle to the same 1e-12 (it is the double oracle that is off there, R30) and number <= 1e-3
+            of the compared set (C10: "report the count and the max");
       FP32  <= 1e-4 per event, <= 1e-6 on the mean of the compared set, no non-finite value.
     The whole batch must be finite and positive and its weights must satisfy w = W * ME (R18).  The printed lines are
     the rows of profiles/r02_parity_full_size.md."""
@@ -476,7 +476,7 @@ def test_full_size_configs_parity(mg, process, prec, n, seed):
             own, res = np.abs(me_o[bad] / me_l - 1), np.abs(me_s[bad] / me_l - 1)
             line += " (vs long double: gpu max %.2e, double oracle's own max %.2e)" % (res.max(), own.max())
             print(line)
-            assert (own > 2.5e-13).all() and (res < 1e-10).all()
+            assert (res <= 1e-12).all()
             assert len(bad) <= max(1, m // 1000)
         else:
             print(line)
