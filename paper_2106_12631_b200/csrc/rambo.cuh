@@ -36,23 +36,36 @@ MG_HD void sincos2pi_(float x, float* s, float* c) {
 MG_HD double log_(double x) { return log(x); }
 MG_HD float log_(float x) { return logf(x); }
 
+// One massless direction and energy from four uniforms (R6): c = 2 rho1 - 1, phi = 2 pi rho2, q0 = -ln(rho3 rho4).
+// The only transcendental part of RAMBO; per particle, so that a kernel may spread it over threads (recycle.cuh, M_GEN).
+template <class T> MG_HD void rambo_direction(T r1, T r2, T r3, T r4, T& q0, T& nx, T& ny, T& nz) {
+  const T c = fma_<T>((T)2, r1, (T)-1);                    // cos(theta) = 2 rho1 - 1
+  const T st = (T)2 * sqrt_<T>(r1 * ((T)1 - r1));          // sqrt(1 - c^2), no cancellation (R19)
+  T sp, cp;
+  sincos2pi_(r2, &sp, &cp);                                 // phi = 2 pi rho2
+  // FP32: the rounded product r3*r4 near 1 would lose the small q0; two logs do not (R19)
+  q0 = sizeof(T) == 8 ? -log_(r3 * r4) : -(log_(r3) + log_(r4));
+  nx = st * cp; ny = st * sp; nz = c;
+}
+
+template <class T, int NF, bool MASSIVE>
+MG_HD T rambo_finish(const T (&q0)[NF], const T (&nx)[NF], const T (&ny)[NF], const T (&nz)[NF], const Consts& k, T (&p)[NF][4]);
+
 // rho[4*i+k] -> p[i][mu] (final particles only); returns the phase-space weight.
 template <class T, int NF, bool MASSIVE>
 MG_HD T rambo_core(const T (&rho)[4 * NF], const Consts& k, T (&p)[NF][4]) {
   T q0[NF], nx[NF], ny[NF], nz[NF];
+#pragma unroll
+  for (int i = 0; i < NF; ++i) rambo_direction<T>(rho[4 * i + 0], rho[4 * i + 1], rho[4 * i + 2], rho[4 * i + 3], q0[i], nx[i], ny[i], nz[i]);
+  return rambo_finish<T, NF, MASSIVE>(q0, nx, ny, nz, k, p);
+}
+
+// boost and scale to (sqrt_s, 0), massive rescaling, weight: everything after the directions
+template <class T, int NF, bool MASSIVE>
+MG_HD T rambo_finish(const T (&q0)[NF], const T (&nx)[NF], const T (&ny)[NF], const T (&nz)[NF], const Consts& k, T (&p)[NF][4]) {
   T Q0 = 0;
 #pragma unroll
-  for (int i = 0; i < NF; ++i) {
-    const T r1 = rho[4 * i + 0], r2 = rho[4 * i + 1], r3 = rho[4 * i + 2], r4 = rho[4 * i + 3];
-    const T c = fma_<T>((T)2, r1, (T)-1);                    // cos(theta) = 2 rho1 - 1
-    const T st = (T)2 * sqrt_<T>(r1 * ((T)1 - r1));          // sqrt(1 - c^2), no cancellation (R19)
-    T sp, cp;
-    sincos2pi_(r2, &sp, &cp);                                 // phi = 2 pi rho2
-    // FP32: the rounded product r3*r4 near 1 would lose the small q0; two logs do not (R19)
-    q0[i] = sizeof(T) == 8 ? -log_(r3 * r4) : -(log_(r3) + log_(r4));
-    nx[i] = st * cp; ny[i] = st * sp; nz[i] = c;
-    Q0 += q0[i];
-  }
+  for (int i = 0; i < NF; ++i) Q0 += q0[i];
   T h[NF][NF];
 #pragma unroll
   for (int i = 0; i < NF; ++i)
@@ -93,17 +106,18 @@ MG_HD T rambo_core(const T (&rho)[4 * NF], const Consts& k, T (&p)[NF][4]) {
   }
   T w = (T)k.w0;
   if (MASSIVE) {
-    // Newton on f(xi) = sum_i sqrt(m_i^2 + xi^2 p_i0^2) - sqrt_s from xi0 = sqrt(1 - (sum m / sqrt_s)^2);
-    // fixed iteration count (lock-step): converged to rounding after 3 steps for the BASELINE masses (R7).
+    // Newton on f(xi) = sum_i sqrt(m_i^2 + xi^2 p_i0^2) - sqrt_s from xi0 = sqrt(1 - (sum m / sqrt_s)^2) (R7).  An event
+    // stops updating once |f| <= 4 eps sqrt_s (its own residual only: the result is a function of the event, not of
+    // the batch); the loop ends when every event of the warp has stopped: 3 updates for the BASELINE masses, at most 8.
     T m2[NF], p02[NF];
     T summ = 0;
 #pragma unroll
     for (int i = 0; i < NF; ++i) { const T m = (T)k.mass[i]; m2[i] = m * m; p02[i] = p[i][0] * p[i][0]; summ += m; }
     const T r = summ / sqrt_s;
     T xi = sqrt_<T>((T)1 - r * r);
-    constexpr int kNewton = sizeof(T) == 8 ? 5 : 4;
+    const T tol = (sizeof(T) == 8 ? (T)8.9e-16 : (T)4.8e-7) * sqrt_s;
 #pragma unroll 1
-    for (int it = 0; it < kNewton; ++it) {
+    for (int it = 0; it < 8; ++it) {
       T f = -sqrt_s, df = 0;
 #pragma unroll
       for (int i = 0; i < NF; ++i) {
@@ -111,7 +125,13 @@ MG_HD T rambo_core(const T (&rho)[4 * NF], const Consts& k, T (&p)[NF][4]) {
         f += E;
         df += xi * p02[i] / E;
       }
-      xi -= f / df;
+      const bool done = abs_<T>(f) <= tol;
+      if (!done) xi -= f / df;
+#ifdef __CUDA_ARCH__
+      if (__all_sync(__activemask(), done)) break;
+#else
+      if (done) break;
+#endif
     }
     T prod = 1, sum2 = 0;
 #pragma unroll

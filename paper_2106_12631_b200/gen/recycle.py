@@ -101,10 +101,12 @@ def _closure_key(c):
 #   BUDGET            entries of new half products per closure chunk
 #   HOIST             producer steps ride with an earlier producer step when that costs no shared memory
 #   HPERM             lane bit i of a thread's index within its event carries the helicity of particle HPERM[i]
+#   ORDER             order of the closure classes (indices into the classes sorted by (helicity bits, kind) of their
+#                     half product); None = sorted
 DEFAULTS = {
-    2: dict(E=8, MINB=3, MINB32=3, EG=None, RELAXED='auto', SLOTS=0, BUDGET=240, HOIST=True, HPERM="2301"),
-    3: dict(E=4, MINB=4, MINB32=5, EG=None, RELAXED='auto', SLOTS=0, BUDGET=240, HOIST=True, HPERM="23104"),
-    4: dict(E=4, MINB=2, MINB32=3, EG=None, RELAXED='auto', SLOTS=424, BUDGET=240, HOIST=True, HPERM="320145"),
+    2: dict(E=8, MINB=3, MINB32=3, EG=None, RELAXED='auto', SLOTS=0, BUDGET=240, HOIST=True, HPERM="2301", ORDER=None),
+    3: dict(E=4, MINB=4, MINB32=5, EG=None, RELAXED='auto', SLOTS=0, BUDGET=240, HOIST=True, HPERM="23104", ORDER=None),
+    4: dict(E=4, MINB=2, MINB32=3, EG=None, RELAXED='auto', SLOTS=424, BUDGET=240, HOIST=True, HPERM="320145", ORDER=(0, 3, 1, 2)),
 }
 
 
@@ -268,6 +270,9 @@ class Program:
             classes.setdefault((nn.nbits, nn.kind), OrderedDict()).setdefault(nn.name, []).append(c)
         chunks, cur, cur_n = [], [], 0
         keys = sorted(classes)
+        if self.opts["ORDER"] is not None:
+            assert sorted(self.opts["ORDER"]) == list(range(len(keys))), keys
+            keys = [keys[i] for i in self.opts["ORDER"]]
         for key in keys:
             names = list(classes[key])
             total = sum(self.half[x].nvar for x in names)
@@ -550,16 +555,27 @@ def emit(prog):
             w("    // step %d: %d inner products" % (si, len(items)))
             cur_b = None
             w("    {")
+            # the operand held in registers across consecutive inner products (B) is the one more closures of the step
+            # share: fewer shared-memory loads per inner product (both products are symmetric in their operands)
+            mult = {}
             for c in items:
+                for x in (c.a, c.b):
+                    mult[x.name] = mult.get(x.name, 0) + 1
+            pairs = []
+            for c in items:
+                held, other = (c.b, c.a) if mult[c.b.name] >= mult[c.a.name] else (c.a, c.b)
+                pairs.append((held, other, c))
+            pairs.sort(key=lambda t: (t[0].name, t[1].name))
+            for held, other, c in pairs:
                 ld_b = "ldv" if c.kind == "DOTV" else "lds"
                 typ = "Vec4<T>" if c.kind == "DOTV" else "Spinor<T>"
-                if c.b.name != cur_b:
+                if held.name != cur_b:
                     if cur_b is not None:
                         w("      }")
-                    w("      { const %s B = ev.%s(%d + rc::pextc<%d>(h));   // %s" % (typ, ld_b, c.b.slot, _hmask(c.b), c.b.name))
-                    cur_b = c.b.name
+                    w("      { const %s B = ev.%s(%d + rc::pextc<%d>(h));   // %s" % (typ, ld_b, held.slot, _hmask(held), held.name))
+                    cur_b = held.name
                 fn = "mdot" if c.kind == "DOTV" else "row_col"
-                w("        { const cx<T> a = %s(ev.%s(%d + rc::pextc<%d>(h)), B);   // %s" % (fn, ld_b, c.a.slot, _hmask(c.a), c.a.name))
+                w("        { const cx<T> a = %s(ev.%s(%d + rc::pextc<%d>(h)), B);   // %s" % (fn, ld_b, other.slot, _hmask(other), other.name))
                 for fl, sg in c.flows:
                     if fl not in seen:
                         seen.add(fl)
