@@ -233,10 +233,15 @@ def stage_rates(mg, torch, r, reps=20):
     kept = torch.empty(n, dtype=torch.int64, device=P.device)
     nkept = [0]
 
-    def unw(i):
-        nkept[0] = len(P.unweight(r["seed"], 0, ew, n, wmax, kept))
-    calls["weight_sums"] = (lambda i: P.weight_sums(ew, n), n * es)
-    calls["unweight"] = (unw, None)
+    d_sums = torch.empty(3, dtype=torch.float64, device=P.device)
+    d_cnt = torch.empty(1, dtype=torch.int64, device=P.device)
+    nkept[0] = len(P.unweight(r["seed"], 0, ew, n, wmax, kept))
+    # device-resident forms (results stay in HBM, no host synchronisation): what a pipeline on the device calls
+    calls["weight_sums"] = (lambda i: P.weight_sums_async(ew, n, d_sums), n * es)
+    calls["unweight"] = (lambda i: P.unweight_async(r["seed"], 0, ew, n, wmax, kept, d_cnt), n * es + 8 * nkept[0])
+    # host-returning forms: the time includes the host round trip
+    calls["weight_sums_sync"] = (lambda i: P.weight_sums(ew, n), n * es)
+    calls["unweight_sync"] = (lambda i: P.unweight(r["seed"], 0, ew, n, wmax, kept), n * es + 8 * nkept[0])
     out = {}
     for name, (fn, stage) in calls.items():
         for i in range(3):
@@ -249,20 +254,14 @@ def stage_rates(mg, torch, r, reps=20):
         b.record()
         torch.cuda.synchronize()
         ms = a.elapsed_time(b) / reps
-        if name == "unweight":
-            stage = 2 * n * es + 8 * nkept[0]            # weights read by the count and the scatter pass, indices written
-            out_extra = {"kept": nkept[0], "of": n}
-        elif stage is None:
+        if stage is None:
             out[name] = {"ms": ms, "MEs_per_s": n / (ms * 1e-3)}
             continue
-        if name in ("weight_sums", "unweight"):          # synchronous calls: the time includes the host round trip
-            gbs = stage / (ms * 1e-3) / 1e9
-            out[name] = {"ms": ms, "GB/s": gbs, "frac_hbm": gbs / hbm if hbm else None, "events_per_s": n / (ms * 1e-3)}
-            if name == "unweight":
-                out[name].update(out_extra)
-            continue
-        gbs = n * P.bytes_per_event(stage) / (ms * 1e-3) / 1e9
+        nbytes = stage if name.startswith(("weight_sums", "unweight")) else n * P.bytes_per_event(stage)
+        gbs = nbytes / (ms * 1e-3) / 1e9
         out[name] = {"ms": ms, "GB/s": gbs, "frac_hbm": gbs / hbm if hbm else None, "events_per_s": n / (ms * 1e-3)}
+        if name.startswith("unweight"):
+            out[name].update({"kept": nkept[0], "of": n})
     return out
 
 

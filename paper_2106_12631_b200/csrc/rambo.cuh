@@ -107,23 +107,26 @@ MG_HD T rambo_finish(const T (&q0)[NF], const T (&nx)[NF], const T (&ny)[NF], co
   T w = (T)k.w0;
   if (MASSIVE) {
     // Newton on f(xi) = sum_i sqrt(m_i^2 + xi^2 p_i0^2) - sqrt_s from xi0 = sqrt(1 - (sum m / sqrt_s)^2) (R7).  An event
-    // stops updating once |f| <= 4 eps sqrt_s (its own residual only: the result is a function of the event, not of
+    // stops updating once |f| <= 16 eps sqrt_s (its own residual only: the result is a function of the event, not of
     // the batch); the loop ends when every event of the warp has stopped: 3 updates for the BASELINE masses, at most 8.
+    // Inside the iteration E_i and 1/E_i come from one reciprocal square root (the iteration corrects its own
+    // rounding); the energies that are stored are recomputed below with a correctly rounded square root.
     T m2[NF], p02[NF];
     T summ = 0;
 #pragma unroll
     for (int i = 0; i < NF; ++i) { const T m = (T)k.mass[i]; m2[i] = m * m; p02[i] = p[i][0] * p[i][0]; summ += m; }
     const T r = summ / sqrt_s;
     T xi = sqrt_<T>((T)1 - r * r);
-    const T tol = (sizeof(T) == 8 ? (T)8.9e-16 : (T)4.8e-7) * sqrt_s;
+    const T tol = (sizeof(T) == 8 ? (T)3.6e-15 : (T)1.9e-6) * sqrt_s;
 #pragma unroll 1
     for (int it = 0; it < 8; ++it) {
       T f = -sqrt_s, df = 0;
 #pragma unroll
       for (int i = 0; i < NF; ++i) {
-        const T E = sqrt_<T>(fma_<T>(xi * xi, p02[i], m2[i]));
-        f += E;
-        df += xi * p02[i] / E;
+        const T arg = fma_<T>(xi * xi, p02[i], m2[i]);
+        const T inv = rsqrt_<T>(arg);
+        f = fma_<T>(arg, inv, f);
+        df = fma_<T>(xi * p02[i], inv, df);
       }
       const bool done = abs_<T>(f) <= tol;
       if (!done) xi -= f / df;

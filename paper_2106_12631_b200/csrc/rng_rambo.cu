@@ -14,6 +14,7 @@ namespace mg {
 namespace {
 
 constexpr int kThreads = 256;
+constexpr int kMinBlocks = 3;      // RAMBO kernels: 24 warps per SM (80 registers) hide the sqrt / division / log chains better than 16 at 124
 
 
 __global__ void __launch_bounds__(kThreads) rng_words_kernel(uint64_t seed, uint64_t first, int64_t n, int64_t ld,
@@ -61,7 +62,7 @@ __device__ __forceinline__ void rambo_event(const T (&rho)[4 * NF], const Consts
 }
 
 template <class T, int NF, bool MASSIVE>
-__global__ void __launch_bounds__(kThreads) rambo_kernel(Consts k, const T* __restrict__ rnd, int64_t n, int64_t ld,
+__global__ void __launch_bounds__(kThreads, kMinBlocks) rambo_kernel(Consts k, const T* __restrict__ rnd, int64_t n, int64_t ld,
                                                          T* __restrict__ mom, T* __restrict__ wout) {
   const int64_t e = (int64_t)blockIdx.x * kThreads + threadIdx.x;
   if (e >= n) return;
@@ -73,7 +74,7 @@ __global__ void __launch_bounds__(kThreads) rambo_kernel(Consts k, const T* __re
 
 // A1-A4 fused: the uniforms stay in registers.
 template <class T, int NF, bool MASSIVE>
-__global__ void __launch_bounds__(kThreads) generate_kernel(Consts k, uint64_t seed, uint64_t first, int64_t n,
+__global__ void __launch_bounds__(kThreads, kMinBlocks) generate_kernel(Consts k, uint64_t seed, uint64_t first, int64_t n,
                                                             int64_t ld, T* __restrict__ mom, T* __restrict__ wout) {
   const int64_t e = (int64_t)blockIdx.x * kThreads + threadIdx.x;
   if (e >= n) return;
