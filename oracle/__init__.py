@@ -5,12 +5,13 @@ __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may 
 package; the product (paper_2106_12631_b200) never does.
 
 Arrays are event-major numpy arrays: rho[n, n_final, 4], mom[n, npar, 4] (E, px, py, pz).
-Process ids: 0 = e+e- -> mu+mu-, 1 = gg -> tt~, 2 = gg -> tt~g, 3 = gg -> tt~gg.
+Process ids: 0 = e+e- -> mu+mu-, 1 = gg -> tt~, 2 = gg -> tt~g, 3 = gg -> tt~gg, 4 = u u~ -> t t~, 5 = u u~ -> t t~ g.
 
 Parity pins (tests/test_oracle_*.py): Philox KAT vectors; RAMBO closed-form weights, momentum
 conservation, on-shellness, 2-body beta/(8 pi); e+e- -> mu+mu- photon+Z closed form and QED limit;
 gg -> tt~ heavy-quark closed form; gauge invariance of every partial amplitude; Lorentz invariance;
-colour-ordered vs colour-dressed brute force; colour-matrix values.  "Event weight" (W_ps * ME) is
+colour-ordered vs colour-dressed brute force; colour-matrix values; u u~ -> t t~ (g): q q~ -> Q Q~ closed form,
+gauge and Lorentz invariance, initial-state collinear limit.  "Event weight" (W_ps * ME) is
 a definition with no independent pin: parity unpinned (reading R18).
 """
 import ctypes as C
@@ -20,9 +21,9 @@ import numpy as np
 
 from .build import build as _build
 
-N_FINAL = {0: 2, 1: 2, 2: 3, 3: 4}
+N_FINAL = {0: 2, 1: 2, 2: 3, 3: 4, 4: 2, 5: 3}
 N_PAR = {k: v + 2 for k, v in N_FINAL.items()}
-DENOM = {0: 4, 1: 256, 2: 256, 3: 512}
+DENOM = {0: 4, 1: 256, 2: 256, 3: 512, 4: 36, 5: 36}
 
 
 class Params(C.Structure):
@@ -120,6 +121,15 @@ def me_dressed(process, mom, par=None, nthreads=0):
     out = np.zeros(n)
     lib().oracle_me_dressed(C.c_int(process), C.byref(par), _p(mom), C.c_int64(n), _p(out), C.c_int(nthreads or hardware_threads()))
     return out
+
+
+def qq_gauge(mom1, par=None):
+    """u u~ -> t t~ g: (largest |M| over colours and helicities with eps -> k/k0, the same with physical polarisations)."""
+    par = par or default_params()
+    mom1 = np.ascontiguousarray(mom1, dtype=np.float64)
+    out = np.zeros(2)
+    lib().oracle_qq_gauge(C.byref(par), _p(mom1), _p(out))
+    return out[0], out[1]
 
 
 def colour_matrix(ng):

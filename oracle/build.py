@@ -6,7 +6,7 @@ import subprocess
 HERE = os.path.dirname(os.path.abspath(__file__))
 LIB = os.path.join(HERE, "liboracle.so")
 SRCS = ["oracle_capi.cpp"]
-DEPS = SRCS + ["common.hpp", "philox.hpp", "rambo.hpp", "dirac.hpp", "me_eemumu.hpp", "me_qcd.hpp"]
+DEPS = SRCS + ["common.hpp", "philox.hpp", "rambo.hpp", "dirac.hpp", "me_eemumu.hpp", "me_qcd.hpp", "me_qq.hpp"]
 
 
 def build(force: bool = False) -> str:

@@ -4,7 +4,7 @@
 // bench.py's cpu_baseline / --impl reference legs can call it through ctypes.  Event-major (AoS)
 // arrays throughout: rho[n][n_final][4], mom[n][npar][4].  Nothing here is used by the product.
 //
-// process ids: 0 = e+e- -> mu+mu-, 1 = gg -> tt~, 2 = gg -> tt~g, 3 = gg -> tt~gg.
+// process ids: 0 = e+e- -> mu+mu-, 1 = gg -> tt~, 2 = gg -> tt~g, 3 = gg -> tt~gg, 4 = u u~ -> t t~, 5 = u u~ -> t t~ g.
 #include <cstdint>
 #include <cstring>
 #include <thread>
@@ -13,12 +13,13 @@
 #include "rambo.hpp"
 #include "me_eemumu.hpp"
 #include "me_qcd.hpp"
+#include "me_qq.hpp"
 
 using namespace oracle;
 
 namespace {
 
-int n_final_of(int process) { return process <= 1 ? 2 : process + 1; }    // 2,2,3,4
+int n_final_of(int process) { return process <= 1 ? 2 : (process <= 3 ? process + 1 : process - 2); }    // 2,2,3,4,2,3
 int n_par_of(int process) { return n_final_of(process) + 2; }
 void masses_of(int process, const Params& par, double* m) {
   int nf = n_final_of(process);
@@ -33,13 +34,14 @@ void me_batch(int process, const Params& par, const double* mom, int64_t n, doub
   int nhel = 1 << np;
   std::vector<T> C;
   QcdProcess P{};
-  if (process >= 1) { P = qcd_process(process + 1); colour_matrix<T>(P.ng, C); }
+  if (process >= 1 && process <= 3) { P = qcd_process(process + 1); colour_matrix<T>(P.ng, C); }
   std::vector<T> hel(nhel);
   for (int64_t e = lo; e < hi; ++e) {
     T p[6][4];
     for (int i = 0; i < np; ++i) for (int mu = 0; mu < 4; ++mu) p[i][mu] = (T)mom[(e * np + i) * 4 + mu];
     T me;
     if (process == 0) me = eemumu_me<T>(par, p, hel.data());
+    else if (process >= 4) me = qq_me<T>(process - 4, par, p, hel.data());
     else me = qcd_me<T>(P, par, C, p, hel.data());
     me_out[e] = (double)me;
     if (hel_out) for (int h = 0; h < nhel; ++h) hel_out[e * nhel + h] = (double)hel[h];
@@ -161,7 +163,7 @@ void oracle_pipeline(int process, const Params* par, uint64_t seed, uint64_t fir
   run_threads(n, nthreads, [=](int64_t lo, int64_t hi) {
     std::vector<double> C;
     QcdProcess P{};
-    if (process >= 1) { P = qcd_process(process + 1); colour_matrix<double>(P.ng, C); }
+    if (process >= 1 && process <= 3) { P = qcd_process(process + 1); colour_matrix<double>(P.ng, C); }
     double masses[4]; masses_of(process, *par, masses);
     for (int64_t e = lo; e < hi; ++e) {
       double rho[16], p[6][4];
@@ -171,9 +173,18 @@ void oracle_pipeline(int process, const Params* par, uint64_t seed, uint64_t fir
       }
       weight[e] = rambo_event<double>(nf, rho, masses, par->sqrt_s, p, 1e-14);
       if (mom_out) for (int i = 0; i < np; ++i) for (int mu = 0; mu < 4; ++mu) mom_out[(e * np + i) * 4 + mu] = p[i][mu];
-      me_out[e] = (process == 0) ? eemumu_me<double>(*par, p) : qcd_me<double>(P, *par, C, p);
+      me_out[e] = (process == 0) ? eemumu_me<double>(*par, p) : (process >= 4 ? qq_me<double>(process - 4, *par, p) : qcd_me<double>(P, *par, C, p));
     }
   });
+}
+
+// u u~ -> t t~ g with the gluon polarisation replaced by its momentum / energy: largest |M| over colour assignments and
+// helicities (out[0]) next to the same with the physical polarisations (out[1])  -- gauge-invariance pin
+void oracle_qq_gauge(const Params* par, const double* mom, double* out) {
+  double p[5][4];
+  for (int i = 0; i < 5; ++i) for (int mu = 0; mu < 4; ++mu) p[i][mu] = mom[i * 4 + mu];
+  qq_me<double>(1, *par, p, nullptr, true, &out[0]);
+  qq_me<double>(1, *par, p, nullptr, false, &out[1]);
 }
 
 int oracle_hardware_threads() { return (int)std::thread::hardware_concurrency(); }
