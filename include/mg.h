@@ -21,7 +21,8 @@
  *        momenta [(i_par  *4 + mu) * ld + e]    mu = 0..3  (E, px, py, pz), GeV
  *        me, ps_weight, event_weight [e]
  *    Particle order (R9): beams first, then the final state as the process is written:
- *        MG_EEMUMU: e+ e- mu+ mu-      MG_GGTT..: g g t t~ [g [g]]
+ *        MG_EEMUMU: e+ e- mu+ mu-      MG_GGTT..: g g t t~ [g [g]]      MG_QQTT, MG_QQTTG: u u~ t t~ [g]  (massless u;
+ *        the quark-initiated channel of SURVEY.md 8(f) N4; its colour basis are the diagrams themselves)
  *    Beams (R5): particle 0 = (sqrt_s/2,0,0,+sqrt_s/2), particle 1 = (sqrt_s/2,0,0,-sqrt_s/2).
  *  - Helicity-combination index: bit k of the index = helicity of particle k (0 <-> -1, 1 <-> +1).
  *  - Determinism: the result for event e depends only on (seed, first_event + e, params), never on
@@ -47,7 +48,7 @@ extern "C" {
 
 typedef struct mg_process mg_process; /* opaque; owns constant tables, two streams and device scratch regions */
 
-enum { MG_EEMUMU = 0, MG_GGTT = 1, MG_GGTTG = 2, MG_GGTTGG = 3 };
+enum { MG_EEMUMU = 0, MG_GGTT = 1, MG_GGTTG = 2, MG_GGTTGG = 3, MG_QQTT = 4, MG_QQTTG = 5 };
 enum { MG_FP64 = 0, MG_FP32 = 1 };
 enum { MG_OK = 0, MG_EINVAL = -1, MG_EPARAM = -2, MG_ECUDA = -3, MG_ENOMEM = -4 };
 /* stages for mg_flops_per_event / mg_bytes_per_event */
@@ -55,7 +56,7 @@ enum { MG_STAGE_RNG = 0, MG_STAGE_RAMBO = 1, MG_STAGE_SIGMAKIN = 2, MG_STAGE_GEN
 
 /* Physics and run parameters (BASELINE.json configs; readings R12-R15). */
 typedef struct {
-  int32_t process;     /* MG_EEMUMU .. MG_GGTTGG */
+  int32_t process;     /* MG_EEMUMU .. MG_QQTTG */
   int32_t precision;   /* MG_FP64 | MG_FP32 */
   int32_t device;      /* CUDA device ordinal */
   int32_t reserved;    /* must be 0 */
@@ -63,8 +64,8 @@ typedef struct {
   double alpha_em_inv; /* 132.507            (MG_EEMUMU) */
   double mZ, gammaZ;   /* 91.188, 2.441 GeV  (MG_EEMUMU) */
   double mW;           /* 80.419 GeV: sin^2(theta_W) = 1 - mW^2/mZ^2 (R14) */
-  double mt;           /* 173 GeV            (MG_GGTT..); the top width is 0 (R12) */
-  double alpha_s;      /* 0.118              (MG_GGTT..) */
+  double mt;           /* 173 GeV            (MG_GGTT.., MG_QQTT..); the top width is 0 (R12) */
+  double alpha_s;      /* 0.118              (MG_GGTT.., MG_QQTT..) */
 } mg_params;
 
 /* Fills *out with the BASELINE.json parameter set for (process, precision), device 0. */

@@ -15,10 +15,10 @@ import torch
 HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(HERE, "libmg_b200.so")
 
-EEMUMU, GGTT, GGTTG, GGTTGG = 0, 1, 2, 3
+EEMUMU, GGTT, GGTTG, GGTTGG, QQTT, QQTTG = 0, 1, 2, 3, 4, 5
 FP64, FP32 = 0, 1
 STAGE_RNG, STAGE_RAMBO, STAGE_SIGMAKIN, STAGE_GENERATE = 0, 1, 2, 3
-PROCESS_NAMES = {"eemumu": EEMUMU, "ggtt": GGTT, "ggttg": GGTTG, "ggttgg": GGTTGG}
+PROCESS_NAMES = {"eemumu": EEMUMU, "ggtt": GGTT, "ggttg": GGTTG, "ggttgg": GGTTGG, "qqtt": QQTT, "qqttg": QQTTG}
 
 
 class MgError(RuntimeError):

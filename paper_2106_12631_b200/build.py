@@ -15,7 +15,7 @@ CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libmg_b200.so")
 PROBE_LIB = os.path.join(HERE, "libmg_probe.so")
-SOURCES = ["mg_api.cu", "rng_rambo.cu", "me_eemumu.cu", "me_ggtt.cu", "me_ggttg.cu", "me_ggttgg.cu", "me_tables.cu", "xsec.cu"]
+SOURCES = ["mg_api.cu", "rng_rambo.cu", "me_eemumu.cu", "me_ggtt.cu", "me_ggttg.cu", "me_ggttgg.cu", "me_qqtt.cu", "me_tables.cu", "xsec.cu"]
 PROBE_SOURCES = ["alu_peak.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "-Xptxas", "-v", "--fmad=true"]

@@ -2,6 +2,7 @@
 #include "mg_internal.h"
 #include "gen_tables.cuh"
 #include "gen_rc_tables.cuh"
+#include "gen_qq_tables.cuh"
 
 namespace mg {
 
@@ -18,6 +19,8 @@ int64_t me_flops_per_helicity(int process) {
     case MG_GGTT: return kFlopsPerHelicity_2;
     case MG_GGTTG: return kFlopsPerHelicity_3;
     case MG_GGTTGG: return kFlopsPerHelicity_4;
+    case MG_QQTT: return kFlopsPerHelicity_qq0;
+    case MG_QQTTG: return kFlopsPerHelicity_qq1;
   }
   return 0;
 }
@@ -27,6 +30,8 @@ int64_t me_flops_per_event_fixed(int process) {
     case MG_GGTT: return kFlopsFixed_2;
     case MG_GGTTG: return kFlopsFixed_3;
     case MG_GGTTGG: return kFlopsFixed_4;
+    case MG_QQTT: return kFlopsFixed_qq0;
+    case MG_QQTTG: return kFlopsFixed_qq1;
   }
   return 0;
 }
@@ -44,6 +49,8 @@ const int* me_colour_numerators(int process, int* den) {
     case MG_GGTT: *den = kColourDen_2; return kColourNum_2;
     case MG_GGTTG: *den = kColourDen_3; return kColourNum_3;
     case MG_GGTTGG: *den = kColourDen_4; return kColourNum_4;
+    case MG_QQTT: *den = kColourDen_qq0; return kColourNum_qq0;
+    case MG_QQTTG: *den = kColourDen_qq1; return kColourNum_qq1;
   }
   return nullptr;
 }

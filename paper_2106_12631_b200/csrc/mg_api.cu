@@ -11,11 +11,13 @@ using namespace mg;
 namespace {
 
 struct ProcInfo { int n_ext, n_final, n_hel, n_flows, n_diag, n_amp, denom; };
-const ProcInfo kInfo[4] = {
+const ProcInfo kInfo[6] = {
     {4, 2, 16, 1, 2, 2, 4},        // e+e- -> mu+mu-     
     {4, 2, 16, 2, 3, 3, 256},      // gg -> tt~          (BASELINE.json configs[2])
     {5, 3, 32, 6, 16, 18, 256},    // gg -> tt~g         (configs[3])
     {6, 4, 64, 24, 123, 159, 512}, // gg -> tt~gg        (configs[4])
+    {4, 2, 16, 1, 1, 1, 36},       // u u~ -> t t~       (quark-initiated channel; diagrams are the colour basis)
+    {5, 3, 32, 5, 5, 5, 36},       // u u~ -> t t~ g
 };
 
 // FP32 handles of g g -> t t~ g (g): events with max |s / propagator denominator| above this go through the
@@ -93,6 +95,8 @@ cudaError_t launch_me(const mg_process* p, const MeArgs& a, cudaStream_t s) {
     case MG_GGTT: return launch_me_ggtt(p, a, s);
     case MG_GGTTG: return launch_me_ggttg(p, a, s);
     case MG_GGTTGG: return launch_me_ggttgg(p, a, s);
+    case MG_QQTT: return launch_me_qqtt(p, a, s);
+    case MG_QQTTG: return launch_me_qqttg(p, a, s);
   }
   return cudaErrorInvalidValue;
 }
@@ -121,7 +125,7 @@ int check_soa(const mg_process* p, const void* ptr, int64_t n, int64_t ld) {
 extern "C" {
 
 int mg_default_params(int process, int precision, mg_params* out) {
-  if (!out || process < 0 || process > 3 || (precision != MG_FP64 && precision != MG_FP32)) return MG_EINVAL;
+  if (!out || process < 0 || process > MG_QQTTG || (precision != MG_FP64 && precision != MG_FP32)) return MG_EINVAL;
   memset(out, 0, sizeof(*out));
   out->process = process; out->precision = precision; out->device = 0;
   out->sqrt_s = 1500.0; out->alpha_em_inv = 132.507; out->mZ = 91.188; out->gammaZ = 2.441; out->mW = 80.419;
@@ -132,7 +136,7 @@ int mg_default_params(int process, int precision, mg_params* out) {
 int mg_init_process(const mg_params* par, mg_process** out) {
   if (!par || !out) return MG_EINVAL;
   *out = nullptr;
-  if (par->process < 0 || par->process > 3 || (par->precision != MG_FP64 && par->precision != MG_FP32) || par->reserved != 0 || par->device < 0)
+  if (par->process < 0 || par->process > MG_QQTTG || (par->precision != MG_FP64 && par->precision != MG_FP32) || par->reserved != 0 || par->device < 0)
     return MG_EINVAL;
   const ProcInfo& I = kInfo[par->process];
   auto pos = [](double x) { return isfinite(x) && x > 0; };
@@ -169,7 +173,7 @@ int mg_init_process(const mg_params* par, mg_process** out) {
   } else {
     k.mass[0] = k.mass[1] = par->mt; k.mt = par->mt;
     k.gs = sqrt(4 * pi * par->alpha_s);                                                // R15
-    const int ng = I.n_ext - 2;
+    const int ng = I.n_ext - 2;                                                        // = number of g_s vertices of every diagram
     k.me_norm = pow(4 * pi * par->alpha_s, ng) / I.denom;                              // g_s^(2 n_g) / denominator
   }
   p->sm_count = prop.multiProcessorCount;
@@ -265,6 +269,8 @@ int mg_sigmakin_fused(mg_process* p, uint64_t seed, uint64_t first_event, int64_
   cudaStream_t s = (cudaStream_t)stream;
   if (p->par.process == MG_EEMUMU) return cuda_rc(launch_fused_eemumu(p, seed, first_event, n, d_me, d_ps_weight, d_event_weight, s));
   if (p->par.process == MG_GGTT) return cuda_rc(launch_fused_ggtt(p, seed, first_event, n, d_me, d_ps_weight, d_event_weight, s));
+  if (p->par.process == MG_QQTT) return cuda_rc(launch_fused_qqtt(p, seed, first_event, n, d_me, d_ps_weight, d_event_weight, s));
+  if (p->par.process == MG_QQTTG) return cuda_rc(launch_fused_qqttg(p, seed, first_event, n, d_me, d_ps_weight, d_event_weight, s));
   // shared-memory kernels: the CTA generates the momenta of its events into shared memory (recycle.cuh, M_GEN)
   MeArgs a{nullptr, n, n, d_me, nullptr, d_event_weight, nullptr, p->hel_mask};
   a.gen = true; a.seed = seed; a.first = first_event; a.psw_out = d_ps_weight;

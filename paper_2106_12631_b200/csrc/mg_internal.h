@@ -72,9 +72,13 @@ cudaError_t launch_me_eemumu(const mg_process* p, const MeArgs& a, cudaStream_t 
 cudaError_t launch_me_ggtt(const mg_process* p, const MeArgs& a, cudaStream_t s);
 cudaError_t launch_me_ggttg(const mg_process* p, const MeArgs& a, cudaStream_t s);
 cudaError_t launch_me_ggttgg(const mg_process* p, const MeArgs& a, cudaStream_t s);
+cudaError_t launch_me_qqtt(const mg_process* p, const MeArgs& a, cudaStream_t s);
+cudaError_t launch_me_qqttg(const mg_process* p, const MeArgs& a, cudaStream_t s);
 // A1-A13 in one kernel (fused.cuh) for the one-thread-per-event processes
 cudaError_t launch_fused_eemumu(const mg_process* p, uint64_t seed, uint64_t first, int64_t n, void* me, void* psw, void* evw, cudaStream_t s);
 cudaError_t launch_fused_ggtt(const mg_process* p, uint64_t seed, uint64_t first, int64_t n, void* me, void* psw, void* evw, cudaStream_t s);
+cudaError_t launch_fused_qqtt(const mg_process* p, uint64_t seed, uint64_t first, int64_t n, void* me, void* psw, void* evw, cudaStream_t s);
+cudaError_t launch_fused_qqttg(const mg_process* p, uint64_t seed, uint64_t first, int64_t n, void* me, void* psw, void* evw, cudaStream_t s);
 // xsec.cu: batch sums of the event weights and hit-or-miss unweighting
 int64_t weight_sums_blocks(int64_t n);
 // d_part: 3 doubles per block of weight_sums_blocks(n); d_out: (sum, sum of squares, max)

@@ -66,3 +66,22 @@ def test_committed_sources_are_current(gens):
 def test_flop_tally_is_positive_and_ordered(gens):
     f = [gens[ng][1].flops_hel for ng in (2, 3, 4)]
     assert 500 < f[0] < f[1] < f[2] < 40000
+
+
+# ----------------------------------------------------------------------------- quark-initiated channel (gen/qqgen.py)
+def test_quark_channel_colour_matrices_and_sources():
+    from paper_2106_12631_b200.gen import qqgen
+    num0, den0 = qqgen.colour_matrix(0)
+    assert num0.tolist() == [[2]] and den0 == 1                       # sum |T^c_ij T^c_lk|^2 = (N^2 - 1)/4
+    num1, den1 = qqgen.colour_matrix(1)
+    K = num1 / den1
+    assert np.allclose(K, K.T) and np.linalg.matrix_rank(K) == 3       # five diagrams, two commutator relations (below)
+    # emission off one line: C_F (N^2 - 1)/4 = 8/3 on the diagonal; three-gluon vertex: N (N^2 - 1)/4 = 6
+    assert np.allclose(np.diag(K), [8 / 3] * 4 + [6])
+    # [T^a, T^c] = i f^{acb} T^b on either line: the three-gluon tensor is the commutator of the two emission tensors
+    C = [c.reshape(-1) for c in qqgen.colour_tensors(1)]
+    assert np.abs(C[0] - C[1] - C[4]).max() < 1e-12 and np.abs(C[3] - C[2] + C[4]).max() < 1e-12
+    src, tables = qqgen.emit()
+    csrc = os.path.join(ROOT, "paper_2106_12631_b200", "csrc")
+    assert open(os.path.join(csrc, "gen_qqtt.cuh")).read() == src, "run python -m paper_2106_12631_b200.gen.qqgen"
+    assert open(os.path.join(csrc, "gen_qq_tables.cuh")).read() == tables

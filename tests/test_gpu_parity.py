@@ -590,3 +590,75 @@ def test_sharded_sums_on_one_device(mg):
     assert abs(mean / one[0] - 1) < 1e-13 and abs(tot[2] / n / one[2] - 1) < 1e-13
     me_o, w_o = oracle.pipeline(2, 7, 100, n)
     assert abs(one[0] / me_o.mean() - 1) < 1e-9 and abs(one[2] / (me_o * w_o).mean() - 1) < 1e-9
+
+
+# ----------------------------------------------------------------------------- quark-initiated channel
+QQ = [4, 5]      # u u~ -> t t~, u u~ -> t t~ g (gen/qqgen.py; oracle/me_qq.hpp pinned in tests/test_oracle_me.py)
+
+
+@pytest.mark.parametrize("prec", [0, 1])
+@pytest.mark.parametrize("process", QQ)
+def test_quark_channel_me_matches_the_oracle(mg, process, prec):
+    """north_star's tolerances, unmodified: FP64 <= 1e-12 per event (events above it against the double oracle are
+    re-compared with the long-double oracle, R30); FP32 <= 1e-4 per event and <= 1e-6 on the batch mean."""
+    n = 16384 + 37
+    P, mom, mom_aos, me_g, me_o = _me_compare(mg, process, prec, n, 7)
+    rel = np.abs(me_g / me_o - 1)
+    assert np.isfinite(me_g).all() and (me_g > 0).all()
+    if prec == 0:
+        bad = np.nonzero(rel > 1e-12)[0]
+        print("quark channel fp64 process %d: n %d, max rel %.2e, above 1e-12: %d" % (process, n, rel.max(), len(bad)))
+        if len(bad):
+            me_l = oracle.me(process, mom_aos[bad], long_double=True)
+            assert (np.abs(me_g[bad] / me_l - 1) <= 1e-12).all() and len(bad) <= n // 1000
+    else:
+        mean_rel = abs(me_g.mean() / me_o.mean() - 1)
+        print("quark channel fp32 process %d: n %d, max rel %.2e, mean rel %.2e" % (process, n, rel.max(), mean_rel))
+        assert rel.max() <= 1e-4 and mean_rel <= 1e-6
+
+
+@pytest.mark.parametrize("process", QQ)
+def test_quark_channel_per_helicity_filter_and_fused_path(mg, process):
+    n = 2048 + 5
+    P = mg.Process(process, 0)
+    assert (P.n_external, P.n_final, P.denominator) == (process, process - 2, 36)
+    mom, w = P.generate(7, 1000, n)
+    hel = _np(P.sigmakin_per_helicity(mom, n), n).T
+    mom_aos = soa_to_aos(_np(mom, n), P.n_external)
+    me_o, hel_o = oracle.me(process, mom_aos, per_helicity=True)
+    coupling = (4 * np.pi * 0.118) ** (P.n_external - 2)
+    assert (np.abs(hel * coupling - hel_o) / hel_o.sum(1, keepdims=True)).max() < 1e-12
+    full = P.sigmakin(mom, n)[:n].clone()
+    mask = P.filter_helicities(mom, 32)
+    # massless u u~ annihilate with opposite helicities only: half of the combinations
+    assert mask == sum(1 << h for h in range(1 << P.n_external) if ((h >> 0) & 1) != ((h >> 1) & 1))
+    assert ((P.sigmakin(mom, n)[:n] / full) - 1).abs().max().item() < 1e-13
+    # A1-A13 in one launch against the oracle's own Philox -> RAMBO -> ME pipeline
+    ew = torch.empty(n, dtype=P.dtype, device=P.device)
+    wf = torch.empty(n, dtype=P.dtype, device=P.device)
+    me_f = P.sigmakin_fused(7, 1000, n, ps_weight=wf, event_weight=ew)
+    me_p, w_p = oracle.pipeline(process, 7, 1000, n)
+    rel = np.abs(me_f.cpu().numpy() / me_p - 1)
+    assert np.median(rel) < 1e-13 and rel.max() < 1e-9 and np.abs(wf.cpu().numpy() / w_p - 1).max() < 1e-9
+    assert torch.equal(ew, wf * me_f)
+    # the colour matrix handed out by the library is the one the kernel uses: K = numerators / denominator of gen/qqgen.py
+    K = P.colour_matrix()
+    assert K.shape == ((1, 1) if process == 4 else (5, 5)) and np.allclose(K, K.T)
+
+
+def test_quark_channel_cross_section_matches_the_closed_form(mg):
+    """sigma(u u~ -> t t~) = (8 pi alpha_s^2 / (27 s)) beta (1 + rho/2), rho = 4 m_t^2 / s (Combridge 1979; the integral of
+    the closed form pinned in tests/test_oracle_me.py): the event weight W_ps * ME of the new channel (R18, R27)."""
+    from oracle import xsec
+    P = mg.Process(4, 0)
+    n = 1 << 18
+    ew = torch.empty(n, dtype=P.dtype, device=P.device)
+    P.sigmakin_fused(7, 0, n, event_weight=ew)
+    s1, s2, mx = P.weight_sums(ew, n)
+    f = xsec.GEV2_TO_PB / (2 * SQRT_S**2)
+    sigma, err = f * s1 / n, f * np.sqrt(max(s2 / n - (s1 / n) ** 2, 0) / n)
+    par = oracle.default_params()
+    rho = 4 * par.mt**2 / SQRT_S**2
+    ref = xsec.GEV2_TO_PB * 8 * np.pi * par.alpha_s**2 / (27 * SQRT_S**2) * np.sqrt(1 - rho) * (1 + rho / 2)
+    print("sigma(u u~ -> t t~) = %.5f +- %.5f pb, closed form %.5f pb" % (sigma, err, ref))
+    assert abs(sigma - ref) < 4 * err and err < 0.01 * ref
