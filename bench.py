@@ -30,15 +30,21 @@ WORKLOADS = {
     "ggttg_fp32": (2, 1, 1 << 21, 7, 3),
     "ggttgg_fp64": (3, 0, 1 << 20, 7, 4),
     "ggttgg_fp32": (3, 1, 1 << 20, 7, 4),
+    # quark-initiated channel (not a BASELINE.json configuration: sized like configs[2] / configs[3])
+    "qqtt_fp64": (4, 0, 1 << 22, 7, None),
+    "qqtt_fp32": (4, 1, 1 << 22, 7, None),
+    "qqttg_fp64": (5, 0, 1 << 21, 7, None),
+    "qqttg_fp32": (5, 1, 1 << 21, 7, None),
 }
-PROC_NAME = {0: "e+ e- -> mu+ mu-", 1: "g g -> t t~", 2: "g g -> t t~ g", 3: "g g -> t t~ g g"}
+PROC_NAME = {0: "e+ e- -> mu+ mu-", 1: "g g -> t t~", 2: "g g -> t t~ g", 3: "g g -> t t~ g g", 4: "u u~ -> t t~", 5: "u u~ -> t t~ g"}
 # CPU-baseline sample sizes: about 10-30 s of oracle work on 8 cores
-CPU_SAMPLE = {0: 1 << 19, 1: 1 << 19, 2: 1 << 16, 3: 1 << 12}
+CPU_SAMPLE = {0: 1 << 19, 1: 1 << 19, 2: 1 << 16, 3: 1 << 12, 4: 1 << 17, 5: 1 << 15}
 # reference arm: events per step (a bounded sample so that steps+warmup end within minutes)
-REF_SAMPLE = {0: 1 << 17, 1: 1 << 17, 2: 1 << 13, 3: 1 << 9}
+REF_SAMPLE = {0: 1 << 17, 1: 1 << 17, 2: 1 << 13, 3: 1 << 9, 4: 1 << 15, 5: 1 << 12}
 # the kernel bench.py brackets with CUDA events for the roofline (what mg_sigmakin launches for that workload)
 KERNEL_NAME = {0: "mg::sigmakin_kernel<mg::Eemumu, %s, false>", 1: "mg::sigmakin_kernel<mg::Ggtt, %s, false>",
-               2: "mg::rc::sigmakin_recycle_kernel<mg::RcGgttg, %s, %s, 0>", 3: "mg::rc::sigmakin_recycle_kernel<mg::RcGgttgg, %s, %s, 0>"}
+               2: "mg::rc::sigmakin_recycle_kernel<mg::RcGgttg, %s, %s, 0>", 3: "mg::rc::sigmakin_recycle_kernel<mg::RcGgttgg, %s, %s, 0>",
+               4: "mg::sigmakin_kernel<mg::Qqtt, %s, false>", 5: "mg::sigmakin_kernel<mg::Qqttg, %s, false>"}
 
 
 def kernel_name(process, prec):
@@ -204,7 +210,7 @@ def time_workload(mg, torch, name, device_index, steps, warmup, dist=None, sampl
     finite = bool(torch.isfinite(me[:n]).all().item())
     flops = P.flops_per_event(mg.STAGE_SIGMAKIN)
     step_bytes = n * (P.bytes_per_event(mg.STAGE_RNG) + P.bytes_per_event(mg.STAGE_RAMBO) + P.bytes_per_event(mg.STAGE_SIGMAKIN))
-    rescued = P.last_rescued() if (prec == 1 and process >= 2) else 0
+    rescued = P.last_rescued() if (prec == 1 and process in (2, 3)) else 0
     return {"P": P, "n": n, "ld": ld, "mask": mask, "total_ms": total_ms, "kern_ms": kern_ms, "mean_me": mean_me, "rescued": rescued,
             "finite": finite, "flops_per_event": flops, "step_bytes": step_bytes, "process": process, "prec": prec,
             "seed": seed, "cfg": cfg, "world": world}
@@ -433,7 +439,7 @@ def main():
                    "paper_baseline": "V100, PAPER.md:116/:159 (context, other hardware)" if args.workload in PAPER_BASELINE else None},
         "e2e": e2e,
         # rng, rambo, sigmaKin per step; FP32 handles of g g -> t t~ g (g) add the double-precision pass over the listed events
-        "gpu_launches": (4 if (prec == 1 and r["process"] >= 2) else 3) * args.steps,
+        "gpu_launches": (4 if (prec == 1 and r["process"] in (2, 3)) else 3) * args.steps,
         "roofline": {"bound": "alu", "kernel": kernel_name(r["process"], prec), "achieved": achieved_tf, "peak": peak_tf, "unit": "TFLOP/s",
                      "frac": achieved_tf / peak_tf, "traffic": None,
                      "flops_per_event": r["flops_per_event"], "kernel_ms": r["kern_ms"],
@@ -464,7 +470,7 @@ def main():
             out["roofline"]["traffic_source"] = ent.get("source")
         else:
             out["roofline"]["traffic_source"] = "no ncu capture of this workload under profiles/"
-        if prec == 1 and r["process"] >= 2:
+        if prec == 1 and r["process"] in (2, 3):
             out["config"]["fp32_events_recomputed_in_double"] = r["rescued"]
     if rank == 0 and world == 1 and not args.no_extra:
         out["cpu_baseline"] = cpu_baseline(r["process"], r["seed"], CPU_SAMPLE[r["process"]])
@@ -481,7 +487,7 @@ def main():
                                "kernel": kernel_name(o["process"], o["prec"]),
                                "alu_frac_of_nominal": tf / pk, "flops_per_event": o["flops_per_event"], "mean_me": o["mean_me"],
                                "all_finite": o["finite"], "stages": stage_rates(mg, torch, o, reps=10)})
-                if o["prec"] == 1 and o["process"] >= 2:
+                if o["prec"] == 1 and o["process"] in (2, 3):
                     others[-1]["fp32_events_recomputed_in_double"] = o["rescued"]
                 if name == "eemumu_16k_fp64":
                     others[-1]["small_batch"] = small_batch_step(mg, torch, o)
