@@ -37,10 +37,10 @@ int64_t me_flops_per_event_fixed(int process) {
 }
 // processes evaluated by the helicity-recycling kernel (recycle.cuh): the tally of everything that kernel
 // executes per event (all helicity variants of every shared wavefunction); -1: per-helicity tally applies
-int64_t me_flops_per_event_recycle(int process) {
+int64_t me_flops_per_event_recycle(int process, bool fp64) {
   switch (process) {
-    case MG_GGTTGG: return kFlopsRecycle_4;
-    case MG_GGTTG: return kFlopsRecycle_3;
+    case MG_GGTTGG: return fp64 ? kFlopsRecycleFp64_4 : kFlopsRecycle_4;
+    case MG_GGTTG: return fp64 ? kFlopsRecycleFp64_3 : kFlopsRecycle_3;
   }
   return -1;
 }

@@ -506,7 +506,7 @@ int mg_last_rescued(mg_process* p, int64_t* h_count_out) {
 int64_t mg_flops_per_event(const mg_process* p, int stage) {
   if (!p) return MG_EINVAL;
   if (stage == MG_STAGE_SIGMAKIN) {
-    const int64_t rc = me_flops_per_event_recycle(p->par.process);
+    const int64_t rc = me_flops_per_event_recycle(p->par.process, p->par.precision == MG_FP64);
     if (rc >= 0) return rc;
     const int good = __builtin_popcountll(p->hel_mask);
     return me_flops_per_event_fixed(p->par.process) + (int64_t)good * me_flops_per_helicity(p->par.process);

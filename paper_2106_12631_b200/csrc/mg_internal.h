@@ -91,7 +91,7 @@ cudaError_t launch_unweight(const mg_process* p, uint64_t seed, uint64_t first, 
 // explicit flop tally of one helicity combination / fixed per-event overhead (generated)
 int64_t me_flops_per_helicity(int process);
 int64_t me_flops_per_event_fixed(int process);
-int64_t me_flops_per_event_recycle(int process);   // >= 0: the process runs the recycling kernel
+int64_t me_flops_per_event_recycle(int process, bool fp64);   // >= 0: the process runs the recycling kernel
 // colour matrix numerators / denominator (generated tables), row-major n_flows x n_flows
 const int* me_colour_numerators(int process, int* denom_out);
 
