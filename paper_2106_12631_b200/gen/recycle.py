@@ -159,9 +159,7 @@ class Program:
             self.mom_names.append(name)
             self.mom_defs.append((tuple(coef), kind))
 
-        for i in range(npar):
-            add("p%d" % i, [1 if j == i else 0 for j in range(npar)], 0)
-
+        # (the external momenta themselves are not in the table: the external wavefunctions read them directly)
         def kcoef(S):
             c = [0] * npar
             for gi in S:

@@ -124,11 +124,11 @@ def run(prog, mom, mt, gs):
                 for v in range(n.nvar):
                     lam = 1 if v else -1
                     if n.kind == "POLVEC":
-                        r = polvec(tab[n.params["mom"]], lam, n.params["outgoing"])
+                        r = polvec(mom[n.params["mom"]], lam, n.params["outgoing"])
                     elif n.kind == "UBAR":
-                        r = bar(spinor_u(tab[n.params["mom"]], mt, lam))
+                        r = bar(spinor_u(mom[n.params["mom"]], mt, lam))
                     elif n.kind == "VSP":
-                        r = spinor_v(tab[n.params["mom"]], mt, lam)
+                        r = spinor_v(mom[n.params["mom"]], mt, lam)
                     elif n.kind == "VCUR":
                         r = np.zeros(4, dtype=complex)
                         for t in n.params["terms"]:

@@ -429,7 +429,8 @@ def _compare_set(process, n):
 
 @pytest.mark.parametrize("process,prec,n,seed", [
     (0, 0, 16384, 42), (0, 0, 1 << 24, 7), (0, 1, 1 << 24, 7), (1, 0, 1 << 22, 7), (1, 1, 1 << 22, 7),
-    (2, 0, 1 << 21, 7), (2, 1, 1 << 21, 7), (3, 0, 1 << 20, 7), (3, 1, 1 << 20, 7)])
+    (2, 0, 1 << 21, 7), (2, 1, 1 << 21, 7), (3, 0, 1 << 20, 7), (3, 1, 1 << 20, 7),
+    (4, 0, 1 << 22, 7), (4, 1, 1 << 22, 7), (5, 0, 1 << 21, 7), (5, 1, 1 << 21, 7)])     # the last four: quark channel, sized like configs 3 and 4
 def test_full_size_configs_parity(mg, process, prec, n, seed):
     """The five configurations of BASELINE.json at their full sizes, in the launch configuration bench.py times
     (mg_rng -> mg_rambo -> mg_filter_helicities -> mg_sigmakin with the event weight), against the oracle fed the GPU's
@@ -481,7 +482,7 @@ def test_full_size_configs_parity(mg, process, prec, n, seed):
         else:
             print(line)
     else:
-        if process >= 2:
+        if process in (2, 3):
             line += "  recomputed in double: %d of %d" % (P.last_rescued(), n)
         print(line)
         assert np.isfinite(me_s).all()
