@@ -33,9 +33,10 @@ KIND_ID = {k: i for i, k in enumerate(KINDS)}
 T_PART, TB_PART = 2, 3
 F_SETUP_MOM = 6 * 4 * 2 + 8 + 2      # one line momentum (6 fma x 4) + Minkowski square + mass shift + reciprocal
 # the same in the FP64 kernels, where the sum is carried as an unevaluated pair and squared exactly (recycle.cuh
-# run_momtab, R30): per component 6 x (1 mul + 6 add) two-sums, 6 for the square, 7 for the accumulation;
-# mass shift 10; final sum and reciprocal 2
-F_SETUP_MOM_DD = 4 * (6 * 7 + 6 + 7) + 10 + 2
+# run_momtab, R30): per component npar x (1 mul + 6 add) two-sums, 6 for the square, 7 for the accumulation;
+# mass shift 10; final sum and reciprocal 2 (npar particles in the sum)
+def f_setup_mom_dd(npar):
+    return 4 * (npar * 7 + 6 + 7) + 10 + 2
 
 
 class RNode:
@@ -416,7 +417,7 @@ class Program:
     def _tally(self):
         self.flops_nodes = sum(n.nvar * n.flops() for n in self.all_nodes)
         self.flops_setup = len(self.mom_defs) * F_SETUP_MOM
-        self.flops_setup_dd = len(self.mom_defs) * F_SETUP_MOM_DD
+        self.flops_setup_dd = len(self.mom_defs) * f_setup_mom_dd(self.npar)
         num, den = self.g.colour_matrix()
         self.num, self.den = num, den
         nf = len(self.g.flows)
