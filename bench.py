@@ -485,7 +485,10 @@ def main():
                 others.append({"workload": name, "value": o["n"] * 3 / (o["total_ms"] * 1e-3), "unit": "MEs/s",
                                "sigmakin_MEs_per_s": o["n"] / (o["kern_ms"] * 1e-3), "sigmakin_ms": o["kern_ms"],
                                "kernel": kernel_name(o["process"], o["prec"]),
-                               "alu_frac_of_nominal": tf / pk, "flops_per_event": o["flops_per_event"], "mean_me": o["mean_me"],
+                               "alu_frac_of_nominal": tf / pk, "flops_per_event": o["flops_per_event"],
+                               # the same launch against the HBM roofline: momenta read, ME / weights written (mg_bytes_per_event)
+                               "sigmakin_hbm_frac": (o["n"] * o["P"].bytes_per_event(mg.STAGE_SIGMAKIN) / (o["kern_ms"] * 1e-3) / 1e9 / peaks["hbm_gbs"]) if peaks.get("hbm_gbs") else None,
+                               "mean_me": o["mean_me"],
                                "all_finite": o["finite"], "stages": stage_rates(mg, torch, o, reps=10)})
                 if o["prec"] == 1 and o["process"] in (2, 3):
                     others[-1]["fp32_events_recomputed_in_double"] = o["rescued"]

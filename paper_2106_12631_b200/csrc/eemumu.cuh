@@ -40,21 +40,10 @@ struct Eemumu {
     a = Ppz * r;
     b = cx<T>(px * r, py * r);
   }
-  // u(p, l): incoming fermion; v(p, l): outgoing antifermion (helas.cuh spinor_u / spinor_v at m = 0)
-  template <class T> static MG_HD Spinor<T> u0(T a, cx<T> b, int l) {
-    Spinor<T> s;
-    const cx<T> z((T)0, (T)0);
-    if (l > 0) { s.l[0] = z; s.l[1] = z; s.r[0] = cx<T>(a, (T)0); s.r[1] = b; }
-    else { s.l[0] = cx<T>(-b.re, b.im); s.l[1] = cx<T>(a, (T)0); s.r[0] = z; s.r[1] = z; }
-    return s;
-  }
-  template <class T> static MG_HD Spinor<T> v0(T a, cx<T> b, int l) {
-    Spinor<T> s;
-    const cx<T> z((T)0, (T)0);
-    if (l > 0) { s.l[0] = cx<T>(-b.re, b.im); s.l[1] = cx<T>(a, (T)0); s.r[0] = z; s.r[1] = z; }
-    else { s.l[0] = z; s.l[1] = z; s.r[0] = cx<T>(-a, (T)0); s.r[1] = -b; }
-    return s;
-  }
+  // helas.cuh spinor_u / spinor_v at m = 0 in terms of (a, b):
+  //   u(p, +) = (0 ; (a, b))        u(p, -) = ((-b^*, a) ; 0)          incoming fermion
+  //   v(p, +) = ((-b^*, a) ; 0)     v(p, -) = (0 ; (-a, -b))           outgoing antifermion
+  //   psibar = (psi_R^* | psi_L^*): the a-block meets psi_R, the b-block meets psi_L
 
   template <class T> static MG_HD void finish(Event<T>& ev, const Consts& k) {
     ev.q = ev.p[0] + ev.p[1];
@@ -68,44 +57,47 @@ struct Eemumu {
     for (int i = 0; i < 4; ++i) massless_frame<T>(ev.p[i], ev.a[i], ev.b[i]);
   }
 
+  // psibar gamma^mu psi of a massless line: only one chirality block of each spinor is non-zero, so the current is ONE of
+  //   R:  J^mu = a sigma^mu psi_R        L:  J^mu = b sigmabar^mu psi_L        (helas.cuh ff_current, one half each)
+  template <class T> static MG_HD Vec4<T> cur_R(cx<T> a0, cx<T> a1, cx<T> r0, cx<T> r1) {
+    const cx<T> a0r0 = a0 * r0, a1r1 = a1 * r1, a0r1 = a0 * r1, a1r0 = a1 * r0;
+    Vec4<T> J;
+    J.v[0] = a0r0 + a1r1; J.v[3] = a0r0 - a1r1; J.v[1] = a0r1 + a1r0; J.v[2] = times_i(a1r0 - a0r1);
+    return J;
+  }
+  template <class T> static MG_HD Vec4<T> cur_L(cx<T> b0, cx<T> b1, cx<T> l0, cx<T> l1) {
+    const cx<T> b0l0 = b0 * l0, b1l1 = b1 * l1, b0l1 = b0 * l1, b1l0 = b1 * l0;
+    Vec4<T> J;
+    J.v[0] = b0l0 + b1l1; J.v[3] = b1l1 - b0l0; J.v[1] = -(b0l1 + b1l0); J.v[2] = times_i(b0l1 - b1l0);
+    return J;
+  }
+
+  // |M|^2 of one helicity combination.  The helicity index is the same for every thread of the launch (the loop over the
+  // good-helicity mask is uniform), so the chirality cases below are uniform branches, not divergence.
+  // Massless leptons: the e+ e- current and the mu+ mu- current vanish unless the two helicities of a line are opposite,
+  // and each is a single chirality block:
+  //   vbar(e+, h0) gamma^mu u(e-, h1):   h1 = +1: a = (-a0, -b0^*), psi_R = (a1, b1)       h1 = -1: b = (-b0, a0), psi_L = (-b1^*, a1)
+  //   ubar(mu-, h3) gamma^mu v(mu+, h2): h3 = +1: a = (a3, b3^*),  psi_R = (-a2, -b2)      h3 = -1: b = (-b3, a3), psi_L = (-b2^*, a2)
+  // (the table above, written out).  With J_e, J_m and the chiral Z couplings g_e, g_m of the two blocks:
+  //   FFV1P0_3 + FFV1_0 :   amp_a = e^2 (J_e . J_m) / s
+  //   FFV2_4_3 + FFV2_4_0:  amp_b = g_e g_m [ (J_e . J_m) - (J_e . q)(J_m . q)/mZ^2 ] / (s - mZ^2 + i mZ GZ)      (R13)
   template <class T> static MG_HD T helicity(const Event<T>& ev, int ihel, const Consts& k) {
-    const int h0 = (ihel & 1) ? 1 : -1, h1 = (ihel & 2) ? 1 : -1, h2 = (ihel & 4) ? 1 : -1, h3 = (ihel & 8) ? 1 : -1;
-    // OXXXXX / IXXXXX: incoming e+ -> vbar, incoming e- -> u, outgoing mu+ -> v, outgoing mu- -> ubar
-    const Spinor<T> vbar_ep = bar(v0<T>(ev.a[0], ev.b[0], h0));
-    const Spinor<T> u_em = u0<T>(ev.a[1], ev.b[1], h1);
-    const Spinor<T> v_mup = v0<T>(ev.a[2], ev.b[2], h2);
-    const Spinor<T> ubar_mum = bar(u0<T>(ev.a[3], ev.b[3], h3));
-    const T e = (T)k.ee, gzl = (T)k.gzl, gzr = (T)k.gzr;
-
-    // chirality-split current of the electron line: J_R = a sigma^mu psi_R, J_L = b sigmabar^mu psi_L
-    Spinor<T> onlyR = vbar_ep, onlyL = vbar_ep;
-    onlyR.r[0] = onlyR.r[1] = cx<T>(0, 0);   // keep a (couples to psi_R)
-    onlyL.l[0] = onlyL.l[1] = cx<T>(0, 0);   // keep b (couples to psi_L)
-    const Vec4<T> JR = ff_current(onlyR, u_em);
-    const Vec4<T> JL = ff_current(onlyL, u_em);
-
-    // FFV1P0_3: A^mu = e (J_L + J_R)^mu / s
-    Vec4<T> A;
-#pragma unroll
-    for (int mu = 0; mu < 4; ++mu) A.v[mu] = (e * ev.is) * (JL.v[mu] + JR.v[mu]);
-    // FFV1_0: e ubar Aslash v
-    const cx<T> amp_a = e * ffv_amp(ubar_mum, A, v_mup);
-
-    // FFV2_4_3: Z^mu = [Jz^mu - q^mu (Jz.q)/mZ^2] / (s - mZ^2 + i mZ GZ),  Jz = gzl J_L + gzr J_R
-    Vec4<T> Jz;
-#pragma unroll
-    for (int mu = 0; mu < 4; ++mu) Jz.v[mu] = rfma(gzr, JR.v[mu], gzl * JL.v[mu]);
-    const cx<T> jq = ((T)1 / (T)k.mZ2) * mdot(Jz, ev.q);
-    Vec4<T> Z;
-#pragma unroll
-    for (int mu = 0; mu < 4; ++mu) Z.v[mu] = ev.bw * rfma(-ev.q.v[mu], jq, Jz.v[mu]);
-    // FFV2_4_0: ubar Zslash (gzl PL + gzr PR) v = gzl b.Sb(Z) v_L + gzr a.S(Z) v_R
-    const Spinor<T> zv = slash_col(slash_parts(Z), v_mup);   // (S(Z) v_R ; Sb(Z) v_L)
-    cx<T> aR = cfma(ubar_mum.l[1], zv.l[1], ubar_mum.l[0] * zv.l[0]);
-    cx<T> bL = cfma(ubar_mum.r[1], zv.r[1], ubar_mum.r[0] * zv.r[0]);
-    const cx<T> amp_b = rfma(gzr, aR, gzl * bL);
-
-    return norm2(amp_a + amp_b);
+    const bool h0 = (ihel & 1) != 0, h1 = (ihel & 2) != 0, h2 = (ihel & 4) != 0, h3 = (ihel & 8) != 0;
+    if (h0 == h1 || h2 == h3) return (T)0;
+    const T a0 = ev.a[0], a1 = ev.a[1], a2 = ev.a[2], a3 = ev.a[3];
+    const cx<T> b0 = ev.b[0], b1 = ev.b[1], b2 = ev.b[2], b3 = ev.b[3];
+    Vec4<T> Je, Jm;
+    T ge, gm;
+    if (h1) { Je = cur_R<T>(cx<T>(-a0, (T)0), -conj_(b0), cx<T>(a1, (T)0), b1); ge = (T)k.gzr; }
+    else { Je = cur_L<T>(-b0, cx<T>(a0, (T)0), -conj_(b1), cx<T>(a1, (T)0)); ge = (T)k.gzl; }
+    if (h3) { Jm = cur_R<T>(cx<T>(a3, (T)0), conj_(b3), cx<T>(-a2, (T)0), -b2); gm = (T)k.gzr; }
+    else { Jm = cur_L<T>(-b3, cx<T>(a3, (T)0), -conj_(b2), cx<T>(a2, (T)0)); gm = (T)k.gzl; }
+    const T e = (T)k.ee;
+    const cx<T> jj = mdot(Je, Jm), jeq = mdot(Je, ev.q), jmq = mdot(Jm, ev.q);
+    const cx<T> zc = (ge * gm) * ev.bw;                                    // Z exchange: couplings x Breit-Wigner
+    const cx<T> coef = cx<T>(fma_<T>(e * e, ev.is, zc.re), zc.im);          // photon + Z on the g^{mu nu} part
+    const cx<T> amp = coef * jj - (zc * ((T)1 / (T)k.mZ2)) * (jeq * jmq);
+    return norm2(amp);
   }
 };
 
