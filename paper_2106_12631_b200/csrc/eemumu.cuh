@@ -20,6 +20,7 @@ namespace mg {
 struct Eemumu {
   static constexpr int NHEL = 16;
   static constexpr int NPAR = 4;
+  static constexpr bool FLIP = false;   // chiral Z couplings: |M(h)|^2 != |M(-h)|^2
 #ifndef MG_EE_MINB
 #define MG_EE_MINB 6
 #endif

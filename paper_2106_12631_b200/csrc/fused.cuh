@@ -38,9 +38,10 @@ __global__ void __launch_bounds__(kMeThreads, Proc::MINB) fused_kernel(Consts k,
   Proc::template finish<T>(ev, k);
   T sum = 0;
 #pragma unroll 1
-  for (uint64_t m = mask; m; m &= m - 1) {
+  for (uint64_t m = flip_half<Proc>(mask); m; m &= m - 1) {
     const int h = __ffsll((long long)m) - 1;
-    sum += Proc::template helicity<T>(ev, h, k);
+    const T v = Proc::template helicity<T>(ev, h, k);
+    sum += Proc::FLIP ? (T)flip_weight<Proc>(mask, h) * v : v;
   }
   const T r = sum * (T)k.me_norm;
   __stcs(me + e, r);

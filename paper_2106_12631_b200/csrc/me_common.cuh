@@ -16,6 +16,21 @@ template <class T> __device__ __forceinline__ Mom<T> load_mom(const T* __restric
 
 constexpr int kMeThreads = 128;
 
+// Helicity-flip symmetry (R35).  For the QCD processes (parity-conserving couplings, tree level, real momenta)
+// the amplitude with every helicity flipped is, up to a sign, the complex conjugate of the original one, so the
+// colour-summed |M|^2 of helicity combination h equals that of its complement NHEL-1-h at the SAME momenta.  Proc::FLIP
+// processes evaluate one member of each pair (the one with the last particle at helicity -1) and count it once per
+// member that the good-helicity mask keeps.  Not for e+ e- -> mu+ mu- (the Z couplings are chiral).
+template <class Proc> MG_HD uint64_t flip_half(uint64_t mask) {
+  if (!Proc::FLIP) return mask;
+  uint64_t rev = 0;
+  for (int h = 0; h < Proc::NHEL / 2; ++h) rev |= ((mask >> (Proc::NHEL - 1 - h)) & 1ull) << h;
+  return (mask | rev) & ((1ull << (Proc::NHEL / 2)) - 1ull);
+}
+template <class Proc> MG_HD int flip_weight(uint64_t mask, int h) {
+  return (int)((mask >> h) & 1ull) + (int)((mask >> (Proc::NHEL - 1 - h)) & 1ull);
+}
+
 // Generic one-thread-per-event kernel.  Proc supplies
 //   struct Event<T> { Mom<T> p[NPAR]; ... }   per-event data that does not depend on the helicity
 //   static void   finish(Event&, consts)      fills the rest of Event from p[]
@@ -34,14 +49,19 @@ __global__ void __launch_bounds__(kMeThreads, Proc::MINB) sigmakin_kernel(Consts
   Proc::template finish<T>(ev, k);
   if (PER_HEL) {
 #pragma unroll 1
-    for (int h = 0; h < Proc::NHEL; ++h) hel_out[(int64_t)h * ld + e] = Proc::template helicity<T>(ev, h, k);
+    for (int h = 0; h < (Proc::FLIP ? Proc::NHEL / 2 : Proc::NHEL); ++h) {
+      const T v = Proc::template helicity<T>(ev, h, k);
+      hel_out[(int64_t)h * ld + e] = v;
+      if (Proc::FLIP) hel_out[(int64_t)(Proc::NHEL - 1 - h) * ld + e] = v;
+    }
     return;
   }
   T sum = 0;
 #pragma unroll 1
-  for (uint64_t m = mask; m; m &= m - 1) {
+  for (uint64_t m = flip_half<Proc>(mask); m; m &= m - 1) {
     const int h = __ffsll((long long)m) - 1;
-    sum += Proc::template helicity<T>(ev, h, k);
+    const T v = Proc::template helicity<T>(ev, h, k);
+    sum += Proc::FLIP ? (T)flip_weight<Proc>(mask, h) * v : v;
   }
   const T r = sum * (T)k.me_norm;
   me[e] = r;

@@ -508,7 +508,14 @@ int64_t mg_flops_per_event(const mg_process* p, int stage) {
   if (stage == MG_STAGE_SIGMAKIN) {
     const int64_t rc = me_flops_per_event_recycle(p->par.process, p->par.precision == MG_FP64);
     if (rc >= 0) return rc;
-    const int good = __builtin_popcountll(p->hel_mask);
+    // helicity combinations the kernel evaluates: the good ones; one of each (h, complement) pair for the QCD processes
+    // (helicity-flip symmetry, me_common.cuh flip_half)
+    int good = __builtin_popcountll(p->hel_mask);
+    if (p->par.process != MG_EEMUMU) {
+      uint64_t half = 0;
+      for (int h = 0; h < p->n_hel / 2; ++h) half |= (((p->hel_mask >> h) | (p->hel_mask >> (p->n_hel - 1 - h))) & 1ull) << h;
+      good = __builtin_popcountll(half);
+    }
     return me_flops_per_event_fixed(p->par.process) + (int64_t)good * me_flops_per_helicity(p->par.process);
   }
   return 0;  // the RNG and RAMBO stages are HBM-bound; their roofline is bytes (mg_bytes_per_event)

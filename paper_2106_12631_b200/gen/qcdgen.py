@@ -378,6 +378,7 @@ class Emitter:
         w("namespace mg {")
         w("struct %s {" % name)
         w("  static constexpr int NHEL = %d;" % (1 << npar))
+        w("  static constexpr bool FLIP = true;    // QCD: |M(h)|^2 = |M(-h)|^2 at fixed momenta (me_common.cuh)")
         w("  static constexpr int MINB = %d;   // resident CTAs of 128 threads the register allocation aims at" % {2: 3}.get(ng, 1))
         w("  static constexpr int NPAR = %d;" % npar)
         w("  static constexpr int NFLOW = %d;" % nf)

@@ -414,3 +414,16 @@ def test_initial_state_collinear_limit_pins_the_normalisation_of_qqttg():
             assert abs(r - 1) < abs(prev - 1)
         prev = r
     assert abs(prev - 1) < 2e-3                                  # linear approach in kT / sqrt(s); a colour or coupling slip is a factor
+
+
+# ----------------------------------------------------------------------------- helicity-flip symmetry (R35)
+def test_helicity_flip_symmetry_holds_for_qcd_and_not_for_the_z():
+    """The QCD kernels evaluate one member of each (h, all helicities flipped) pair and count it twice.  That rests on
+    |M(h)|^2 = |M(-h)|^2 at FIXED momenta (tree level, parity-conserving couplings, real momenta: M(-h) = +- M(h)^*); the
+    oracle, which evaluates every helicity combination from the plain definition, must show it — and must show that it
+    fails for e+ e- -> mu+ mu- (chiral Z couplings), where the kernels do not use it."""
+    for process, n in ((1, 16), (2, 8), (3, 3), (4, 16), (5, 8)):
+        me, hel = oracle.me(process, _events(process, n), per_helicity=True)
+        assert (np.abs(hel - hel[:, ::-1]) / hel.sum(1, keepdims=True)).max() < 1e-14, process
+    me, hel = oracle.me(0, _events(0, 16, seed=42), per_helicity=True)
+    assert (np.abs(hel - hel[:, ::-1]) / hel.sum(1, keepdims=True)).max() > 1e-2
