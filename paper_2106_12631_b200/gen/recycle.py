@@ -106,12 +106,17 @@ def _closure_key(c):
 #   BUDGET            entries of new half products per closure chunk
 #   HOIST             producer steps ride with an earlier producer step when that costs no shared memory
 #   HPERM             lane bit i of a thread's index within its event carries the helicity of particle HPERM[i]
+#   FLIP              helicity-flip symmetry (R35): the last particle's helicity is fixed at -1, one thread per
+#                     combination of the OTHER helicities; |M|^2 counts for the combination and its complement
 #   ORDER             order of the closure classes (indices into the classes sorted by (helicity bits, kind) of their
 #                     half product); None = sorted
 DEFAULTS = {
-    2: dict(E=8, MINB=3, MINB32=3, EG=None, RELAXED='auto', SLOTS=0, BUDGET=240, HOIST=True, HPERM="2301", ORDER=None),
-    3: dict(E=4, MINB=4, MINB32=5, EG=None, RELAXED='auto', SLOTS=0, BUDGET=240, HOIST=True, HPERM="23104", ORDER=None),
-    4: dict(E=4, MINB=2, MINB32=3, EG=None, RELAXED='auto', SLOTS=424, BUDGET=240, HOIST=True, HPERM="320145", ORDER=(0, 3, 1, 2)),
+    2: dict(E=8, MINB=3, MINB32=3, EG=None, RELAXED='auto', SLOTS=0, BUDGET=240, HOIST=True, HPERM="2301", ORDER=None, FLIP=False),
+    # FLIP (round 2): one warp (g g -> t t~ g g) / half a warp (g g -> t t~ g) per event, 16 / 32 events per SM.  Without it the
+    # tuned shapes were E=4, MINB=4/5, HPERM="23104" and E=4, MINB=2/3, SLOTS=424, HPERM="320145", ORDER=(0, 3, 1, 2)
+    # (27.2 ms per 2^20 g g -> t t~ g g events against 17.5 ms; shapes timed: profiles/r02_h_*)
+    3: dict(E=8, MINB=4, MINB32=5, EG=None, RELAXED='auto', SLOTS=0, BUDGET=240, HOIST=True, HPERM="2310", ORDER=None, FLIP=True),
+    4: dict(E=8, MINB=2, MINB32=3, EG=None, RELAXED='auto', SLOTS=0, BUDGET=96, HOIST=True, HPERM="32014", ORDER=None, FLIP=True),
 }
 
 
@@ -121,7 +126,6 @@ class Program:
         self.ng = ng
         g = self.g = qcdgen.Generator(ng)
         self.npar = ng + 2
-        self.nhel = 1 << self.npar
         o = dict(DEFAULTS[ng])
         assert set(opts) <= set(o), opts
         o.update(opts)
@@ -131,6 +135,9 @@ class Program:
         assert self.E % self.EG == 0
         self.RELAXED = o["RELAXED"]
         self.SLOT_LIMIT = o["SLOTS"]
+        self.flip = bool(o["FLIP"])
+        self.fixed = self.npar - 1 if self.flip else None       # particle whose helicity is not a thread index bit
+        self.nhel = 1 << (self.npar - (1 if self.flip else 0))    # threads per event
         self.NT = self.E * self.nhel
         self.gp = g.gl_particle
         self._build_momenta()
@@ -200,7 +207,7 @@ class Program:
             return n
 
         for gi in range(self.ng):
-            add(RNode("eps%d" % gi, "POLVEC", [self.gp[gi]], mom=self.gp[gi], outgoing=gi >= 2))
+            add(RNode("eps%d" % gi, "POLVEC", [p for p in [self.gp[gi]] if p != self.fixed], mom=self.gp[gi], outgoing=gi >= 2))
         add(RNode("ubar", "UBAR", [T_PART], mom=T_PART))
         add(RNode("v", "VSP", [TB_PART], mom=TB_PART))
         for st in g.struct_order:
@@ -225,7 +232,7 @@ class Program:
                 # every structure is (X.Y) Z - (Z.Y) X after a permutation (csrc/recycle.cuh vvvv_acc)
                 cops = {1: [ops[0], ops[2], ops[1]], 2: ops, 3: [ops[1], ops[0], ops[2]]}[which]
                 out.append(dict(type=which, sign=t[0], ops=ops, cops=cops, momA=0, momB=0))
-        return RNode(name, "VCUR", [self.gp[gi] for gi in subset], terms=out, prop=prop)
+        return RNode(name, "VCUR", [self.gp[gi] for gi in subset if self.gp[gi] != self.fixed], terms=out, prop=prop)
 
     # ------------------------------------------------------------------ closures as inner products
     def _build_closures(self):
@@ -515,12 +522,16 @@ def emit(prog):
     w("};")
     w("struct %s {" % name)
     w("  static constexpr int NPAR = %d, NHEL = %d, NFLOW = %d, E = %d, EG = %d, NT = %d, NTG = %d, MINB = %d, MINB32 = %d;" % (npar, prog.nhel, nf, prog.E, prog.EG, prog.NT, prog.EG * prog.nhel, prog.MINB, prog.MINB32))
+    w("  // NHEL = threads per event.  FLIP: the helicity of the last particle is fixed at -1 and every |M|^2 counts for the")
+    w("  // combination and its complement (|M(h)|^2 = |M(-h)|^2 at fixed momenta, DESIGN.md R35); NBITS = helicity bits in a thread index")
+    w("  static constexpr bool FLIP = %s;" % ("true" if prog.flip else "false"))
+    w("  static constexpr int NHEL_FULL = %d, NBITS = %d;" % (1 << npar, npar - (1 if prog.flip else 0)))
     w("  static constexpr int NMOM = %d, NSLOT = %d;" % (len(prog.mom_defs), prog.nslot))
     # lane bit i of a thread's index within its event carries the helicity of particle hperm[i]: t and t~ in the two
     # lowest bits.  All 720 / 120 orders were timed on B200 with a run-time permutation, the best few rebuilt with the
     # compile-time one: 2.7 % (g g -> t t~ g g) and 2 % (g g -> t t~ g) faster than particle order
     hperm = prog.opts["HPERM"]
-    assert sorted(hperm) == [str(i) for i in range(npar)]
+    assert sorted(hperm) == [str(i) for i in range(npar) if i != prog.fixed]
     w("  static constexpr unsigned HPERM = 0x%s;   // nibble i: particle whose helicity is bit i of the lane index" % hperm[::-1])
     w("  static __device__ __forceinline__ const rc::NodeDesc& node(int i) { return kRcNode_%s[i]; }" % tag)
     w("  static __device__ __forceinline__ const rc::TermDesc& term(int i) { return kRcTerm_%s[i]; }" % tag)

@@ -172,4 +172,5 @@ def run(prog, mom, mt, gs):
     C = prog.num / prog.den
     per_hel = np.einsum("hf,fg,hg->h", jamp.conj(), C, jamp).real
     denom = {2: 256, 3: 256, 4: 512}[prog.ng]
-    return per_hel.sum() * gs ** (2 * prog.ng) / denom, per_hel
+    # FLIP programs carry one member of every (h, complement) pair of helicity combinations: each counts twice
+    return (2 if getattr(prog, "flip", False) else 1) * per_hel.sum() * gs ** (2 * prog.ng) / denom, per_hel

@@ -65,7 +65,7 @@ def test_program_shape(programs):
     # 3 / 15 / 105 inner products once diagrams that differ only in a gluon sub-tree share an off-shell current
     assert [len(programs[ng].closures) for ng in (2, 3, 4)] == [3, 15, 105]
     for ng, prog in programs.items():
-        assert prog.nhel == 1 << (ng + 2)
+        assert prog.nhel == 1 << (ng + 2 - (1 if prog.flip else 0))       # threads per event (FLIP: the last helicity is fixed)
         # every node is written before it is read and its slots lie inside the allocated entries
         for n in prog.all_nodes:
             assert n.born < n.last and n.slot + n.nvar <= prog.nslot
