@@ -55,6 +55,9 @@ def kernel_name(process, prec):
 
 PAPER_BASELINE = {"ggttgg_fp64": 5e5, "eemumu_fp64": 1.37e9, "eemumu_fp32": 3.28e9}   # V100
 
+# flop tallies of the shared-memory kernels before the helicity-flip symmetry (commit b02c00b: gen_rc_tables.cuh), (process, precision)
+FULL_SUM_FLOPS = {(3, 0): 503313, (3, 1): 498267, (2, 0): 40333, (2, 1): 38435}
+
 # FP64 / FP32 FMA lanes per SM; peak = 148 SMs x lanes x 2 x sm clock
 LANES = {0: 64, 1: 128}
 
@@ -444,7 +447,14 @@ def main():
                      "frac": achieved_tf / peak_tf, "traffic": None,
                      "flops_per_event": r["flops_per_event"], "kernel_ms": r["kern_ms"],
                      "peak_kind": "nominal (lanes x clock); the measured_* entries are on-box microbenchmarks of the same pipe",
-                     "peak_source": "148 SMs x %d FMA lanes x 2 x %.0f MHz (MEASURED_PEAKS.json sm_max_mhz)" % (LANES[prec], sm_max)},
+                     "peak_source": "148 SMs x %d FMA lanes x 2 x %.0f MHz (MEASURED_PEAKS.json sm_max_mhz)" % (LANES[prec], sm_max),
+                     # frac counts the flops this kernel EXECUTES.  The QCD kernels use |M(h)|^2 = |M(-h)|^2 (R35): they
+                     # evaluate half of the helicity combinations.  For context, the same launch against the flop count of the
+                     # same algorithm WITHOUT that symmetry (round-2 kernel before it: 503 313 flop per g g -> t t~ g g event at
+                     # 27.4 ms = 0.518 of the peak): not a fraction of executed work, never the headline
+                     "flops_per_event_full_helicity_sum": FULL_SUM_FLOPS.get((r["process"], prec)),
+                     "frac_vs_full_helicity_sum_flops": (FULL_SUM_FLOPS[(r["process"], prec)] * n / (r["kern_ms"] * 1e-3) / 1e12 / peak_tf)
+                     if (r["process"], prec) in FULL_SUM_FLOPS else None},
         "mean_me": r["mean_me"], "all_finite": r["finite"],
     }
     if rank == 0:
