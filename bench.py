@@ -234,6 +234,10 @@ def stage_rates(mg, torch, r, reps=20):
     ew = torch.empty(ld, dtype=P.dtype, device=P.device)
     # A1-A13 in one call, momenta never stored: whole-path MEs/s next to the three-kernel step
     calls["fused_path"] = (lambda i: P.sigmakin_fused(r["seed"], i * n, n, me, w, ew), None)
+    # sigmaKin alone, next to its two-kernel form under a CUDA graph: same momenta, same values
+    if r["process"] in (2, 3):
+        calls["sigmakin"] = (lambda i: P.sigmakin(mom, n, me), None)
+        calls["sigmakin_split_graph"] = (lambda i: P.sigmakin_split(mom, n, me=me), None)
     # after the path: batch sums of the event weights and hit-or-miss stream compaction
     fn_f = calls["fused_path"][0]
     fn_f(0)

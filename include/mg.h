@@ -120,6 +120,22 @@ int mg_generate(mg_process* p, uint64_t seed, uint64_t first_event, int64_t n, i
 int mg_sigmakin_fused(mg_process* p, uint64_t seed, uint64_t first_event, int64_t n,
                       void* d_me, void* d_ps_weight, void* d_event_weight, void* stream);
 
+/* A5-A13 as TWO kernels per chunk of events under a CUDA graph (§5, the third remedy
+ * for the register pressure of sigmaKin: "splitting the SIGMAKIN kernel into many smaller kernels ... orchestrated by
+ * CUDA graphs").  Same arguments and the same values, bit for bit, as mg_sigmakin of the same handle; only
+ * MG_GGTTG and MG_GGTTGG (the shared-memory kernels), MG_EINVAL otherwise.  Kernel A of a chunk evaluates the
+ * amplitudes and writes the colour-flow sums J_f of every evaluated helicity combination to device scratch of the
+ * handle; kernel B reads them back and does the colour sum, the helicity sum and the averaging.  The n events are cut
+ * into chunks of chunk_events (a positive multiple of 8; 0 = the library's choice, 16 384); chunk c runs on branch
+ * c % 2 of the graph with its own scratch, so that B of one chunk overlaps A of the next.  The graph is built on the first call and kept in the handle; it is rebuilt when
+ * any argument other than `stream`, or the helicity mask, changes.  FP32 handles: the double-precision pass over the
+ * ill-conditioned events (mg_set_fp32_rescue) is NOT part of this path; the values are those of mg_sigmakin with the
+ * pass switched off.  This is the measured alternative, not the default: DESIGN.md §7.2 has the numbers.
+ * Scratch: 2 * chunk_events * 2^(n_external-1) * n_colour_flows complex numbers.  Asynchronous on `stream`.
+ * Errors: MG_EINVAL, MG_ENOMEM, MG_ECUDA. */
+int mg_sigmakin_split(mg_process* p, const void* d_momenta, int64_t n, int64_t ld, void* d_me,
+                      const void* d_ps_weight, void* d_event_weight, int64_t chunk_events, void* stream);
+
 /* After the hot path ("a fiducial cross section ... and a sample of N_unw unweighted
  * events", "event unweighting, where data stream compaction should in principle be straight-forward").
  *

@@ -62,6 +62,7 @@ def lib():
         "mg_sigmakin": (C.c_int, [vp, vp, i64, i64, vp, vp, vp, vp]),
         "mg_sigmakin_per_helicity": (C.c_int, [vp, vp, i64, i64, vp, vp]),
         "mg_sigmakin_fused": (C.c_int, [vp, u64, u64, i64, vp, vp, vp, vp]),
+        "mg_sigmakin_split": (C.c_int, [vp, vp, i64, i64, vp, vp, vp, i64, vp]),
         "mg_weight_sums": (C.c_int, [vp, vp, i64, C.POINTER(C.c_double), vp]),
         "mg_unweight": (C.c_int, [vp, u64, u64, vp, i64, C.c_double, vp, C.POINTER(i64), vp]),
         "mg_sigmakin_host": (C.c_int, [vp, vp, i64, i64, vp]),
@@ -87,7 +88,7 @@ def lib():
 EXPORTED = ["mg_default_params", "mg_init_process", "mg_free_process", "mg_n_external", "mg_n_final", "mg_n_helicities",
             "mg_n_colour_flows", "mg_n_diagrams", "mg_n_amplitudes", "mg_me_denominator", "mg_colour_matrix",
             "mg_padded_stride", "mg_rng_words", "mg_rng", "mg_rambo", "mg_generate", "mg_filter_helicities",
-            "mg_set_helicity_mask", "mg_get_helicity_mask", "mg_sigmakin", "mg_sigmakin_per_helicity", "mg_sigmakin_fused", "mg_weight_sums", "mg_unweight",
+            "mg_set_helicity_mask", "mg_get_helicity_mask", "mg_sigmakin", "mg_sigmakin_per_helicity", "mg_sigmakin_fused", "mg_sigmakin_split", "mg_weight_sums", "mg_unweight",
             "mg_sigmakin_host", "mg_run_host", "mg_flops_per_event", "mg_bytes_per_event", "mg_last_kernel_ms",
             "mg_weight_sums_async", "mg_unweight_async", "mg_set_fp32_rescue", "mg_get_fp32_rescue", "mg_last_rescued",
             "mg_strerror", "mg_version"]
@@ -198,6 +199,14 @@ class Process:
         ld = momenta.shape[1]
         me = me if me is not None else torch.empty(ld, dtype=self.dtype, device=self.device)
         _check(lib().mg_sigmakin(self._h, _ptr(momenta), n, ld, _ptr(me), _ptr(ps_weight), _ptr(event_weight), _stream(self.device)))
+        return me
+
+    def sigmakin_split(self, momenta, n, me=None, ps_weight=None, event_weight=None, chunk_events=0):
+        """mg_sigmakin_split: the same values as sigmakin from two kernels per chunk of events under a CUDA graph."""
+        ld = momenta.shape[1]
+        me = me if me is not None else torch.empty(ld, dtype=self.dtype, device=self.device)
+        _check(lib().mg_sigmakin_split(self._h, _ptr(momenta), n, ld, _ptr(me), _ptr(ps_weight), _ptr(event_weight),
+                                       chunk_events, _stream(self.device)))
         return me
 
     def sigmakin_per_helicity(self, momenta, n, out=None):

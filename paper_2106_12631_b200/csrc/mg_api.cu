@@ -182,7 +182,9 @@ int mg_init_process(const mg_params* par, mg_process** out) {
   bool ok = g.ok && cudaStreamCreateWithFlags(&p->own_stream, cudaStreamNonBlocking) == cudaSuccess &&
             cudaStreamCreateWithFlags(&p->own_stream2, cudaStreamNonBlocking) == cudaSuccess &&
             cudaEventCreate(&p->ev0) == cudaSuccess && cudaEventCreate(&p->ev1) == cudaSuccess &&
-            scratch_init(p->sc_host) && scratch_init(p->sc_xsec) && scratch_init(p->sc_rescue[0]) && scratch_init(p->sc_rescue[1]);
+            scratch_init(p->sc_host) && scratch_init(p->sc_xsec) && scratch_init(p->sc_rescue[0]) && scratch_init(p->sc_rescue[1]) && scratch_init(p->sc_split) &&
+            cudaEventCreateWithFlags(&p->split_fork, cudaEventDisableTiming) == cudaSuccess &&
+            cudaEventCreateWithFlags(&p->split_join, cudaEventDisableTiming) == cudaSuccess;
   for (int i = 0; ok && i < 16; ++i) ok = cudaEventCreate(&p->kev[i]) == cudaSuccess;
   if (!ok) { cudaGetLastError(); mg_free_process(p); return MG_ECUDA; }
   *out = p;
@@ -193,6 +195,10 @@ int mg_free_process(mg_process* p) {
   if (!p) return MG_OK;
   DeviceGuard g(p->par.device);
   scratch_free(p->sc_host); scratch_free(p->sc_xsec); scratch_free(p->sc_rescue[0]); scratch_free(p->sc_rescue[1]);
+  scratch_free(p->sc_split);                      // waits for the last graph launch
+  if (p->split_exec) cudaGraphExecDestroy(p->split_exec);
+  if (p->split_fork) cudaEventDestroy(p->split_fork);
+  if (p->split_join) cudaEventDestroy(p->split_join);
   for (int i = 0; i < 16; ++i) if (p->kev[i]) cudaEventDestroy(p->kev[i]);
   if (p->ev0) cudaEventDestroy(p->ev0);
   if (p->ev1) cudaEventDestroy(p->ev1);
@@ -258,6 +264,63 @@ int mg_sigmakin(mg_process* p, const void* d_momenta, int64_t n, int64_t ld, voi
   DeviceGuard g(p->par.device); if (!g.ok) return MG_ECUDA;
   p->rescue_last_mask = 0;
   return run_me(p, a, (cudaStream_t)stream, 0);
+}
+
+// mg_sigmakin_split: see include/mg.h and csrc/split.cuh
+int mg_sigmakin_split(mg_process* p, const void* d_momenta, int64_t n, int64_t ld, void* d_me, const void* d_ps_weight, void* d_event_weight,
+                      int64_t chunk_events, void* stream) {
+  int rc = check_soa(p, d_momenta, n, ld); if (rc != MG_OK) return rc;
+  if (!shared_memory_kernel(p) || chunk_events < 0 || chunk_events % 8 != 0) return MG_EINVAL;
+  if (n == 0) return MG_OK;
+  if (!d_me || !aligned(d_me, elem(p))) return MG_EINVAL;
+  const bool gg = p->par.process == MG_GGTTGG;
+  DeviceGuard g(p->par.device); if (!g.ok) return MG_ECUDA;
+  cudaStream_t s = (cudaStream_t)stream;
+  if (cuda_rc(gg ? prepare_split_ggttgg(p) : prepare_split_ggttg(p)) != MG_OK) { cudaGetLastError(); return MG_ECUDA; }
+  // default chunk: measured on B200 (chunks of 1 184 .. 262 144 events): chunks whose J_f stay in the L2
+  // (6 / 12 KB per event in FP64) lose more to the tails of their short launches than they save in HBM traffic
+  int64_t chunk = chunk_events ? chunk_events : 16384;
+  if (chunk > n) chunk = (n + 7) / 8 * 8;
+  const size_t per_branch = ((gg ? split_scratch_bytes_ggttgg(p, chunk) : split_scratch_bytes_ggttg(p, chunk)) + 255) / 256 * 256;
+  const void* psw = (d_ps_weight && d_event_weight) ? d_ps_weight : nullptr;
+  void* evw = psw ? d_event_weight : nullptr;
+  rc = acquire(p->sc_split, 2 * per_branch, s); if (rc != MG_OK) return rc;
+  auto& key = p->split_key;
+  const bool same = p->split_exec && key.mom == d_momenta && key.n == n && key.ld == ld && key.me == d_me && key.psw == psw && key.evw == evw &&
+                    key.chunk == chunk && key.mask == p->hel_mask && key.scratch == p->sc_split.d;
+  if (!same) {
+    if (p->split_exec) {
+      if (p->sc_split.used) cudaEventSynchronize(p->sc_split.done);       // the old graph may still be running
+      cudaGraphExecDestroy(p->split_exec); p->split_exec = nullptr;
+    }
+    // capture: fork own_stream -> own_stream2, chunk c on branch c % 2 (kernel A, kernel B, its own half of the scratch), join
+    cudaStream_t br[2] = {p->own_stream, p->own_stream2};
+    const size_t es = elem(p);
+    cudaGraph_t graph = nullptr;
+    cudaError_t e = cudaStreamBeginCapture(br[0], cudaStreamCaptureModeThreadLocal);
+    if (e == cudaSuccess) e = cudaEventRecord(p->split_fork, br[0]);
+    if (e == cudaSuccess) e = cudaStreamWaitEvent(br[1], p->split_fork, 0);
+    int64_t c = 0;
+    for (int64_t c0 = 0; e == cudaSuccess && c0 < n; c0 += chunk, ++c) {
+      const int64_t width = n - c0 < chunk ? n - c0 : chunk;
+      MeArgs a{(const char*)d_momenta + (size_t)c0 * es, width, ld, (char*)d_me + (size_t)c0 * es,
+               psw ? (const char*)psw + (size_t)c0 * es : nullptr, evw ? (char*)evw + (size_t)c0 * es : nullptr, nullptr, p->hel_mask};
+      void* jamp = (char*)p->sc_split.d + (size_t)(c & 1) * per_branch;
+      e = gg ? launch_split_chunk_ggttgg(p, a, jamp, br[c & 1]) : launch_split_chunk_ggttg(p, a, jamp, br[c & 1]);
+    }
+    if (e == cudaSuccess) e = cudaEventRecord(p->split_join, br[1]);
+    if (e == cudaSuccess) e = cudaStreamWaitEvent(br[0], p->split_join, 0);
+    const cudaError_t e2 = cudaStreamEndCapture(br[0], &graph);           // always ends the capture, also after an error
+    if (e == cudaSuccess) e = e2;
+    if (e == cudaSuccess) e = cudaGraphInstantiate(&p->split_exec, graph, 0);
+    if (graph) cudaGraphDestroy(graph);
+    if (e != cudaSuccess) { cudaGetLastError(); p->split_exec = nullptr; return cuda_rc(e); }
+    key.mom = d_momenta; key.n = n; key.ld = ld; key.me = d_me; key.psw = psw; key.evw = evw; key.chunk = chunk; key.mask = p->hel_mask;
+    key.scratch = p->sc_split.d;
+  }
+  const cudaError_t e = cudaGraphLaunch(p->split_exec, s);
+  rc = release(p->sc_split, s);
+  return e != cudaSuccess ? cuda_rc(e) : rc;
 }
 
 int mg_sigmakin_fused(mg_process* p, uint64_t seed, uint64_t first_event, int64_t n, void* d_me, void* d_ps_weight, void* d_event_weight, void* stream) {

@@ -36,6 +36,12 @@ struct mg_process {
   cudaEvent_t ev0, ev1;
   cudaEvent_t kev[16];                    // start/end of the sigmaKin launch of each chunk of a host call
   double last_kernel_ms;
+  // mg_sigmakin_split: the instantiated graph, the arguments it was captured for, its scratch (two branches) and the
+  // fork/join events of the capture
+  mg_scratch sc_split;
+  cudaGraphExec_t split_exec;
+  struct { const void* mom; int64_t n, ld; void* me; const void* psw; void* evw; int64_t chunk; uint64_t mask; void* scratch; } split_key;
+  cudaEvent_t split_fork, split_join;
 };
 
 namespace mg {
@@ -74,6 +80,14 @@ cudaError_t launch_me_ggttg(const mg_process* p, const MeArgs& a, cudaStream_t s
 cudaError_t launch_me_ggttgg(const mg_process* p, const MeArgs& a, cudaStream_t s);
 cudaError_t launch_me_qqtt(const mg_process* p, const MeArgs& a, cudaStream_t s);
 cudaError_t launch_me_qqttg(const mg_process* p, const MeArgs& a, cudaStream_t s);
+// split.cuh: the two-kernel form of the shared-memory processes (mg_sigmakin_split): attributes of kernel A (outside a
+// capture), J scratch of one chunk, kernels A and B of one chunk (a = the chunk's slice of the caller's arrays)
+cudaError_t prepare_split_ggttg(const mg_process* p);
+cudaError_t prepare_split_ggttgg(const mg_process* p);
+size_t split_scratch_bytes_ggttg(const mg_process* p, int64_t chunk);
+size_t split_scratch_bytes_ggttgg(const mg_process* p, int64_t chunk);
+cudaError_t launch_split_chunk_ggttg(const mg_process* p, const MeArgs& a, void* jamp, cudaStream_t s);
+cudaError_t launch_split_chunk_ggttgg(const mg_process* p, const MeArgs& a, void* jamp, cudaStream_t s);
 // A1-A13 in one kernel (fused.cuh) for the one-thread-per-event processes
 cudaError_t launch_fused_eemumu(const mg_process* p, uint64_t seed, uint64_t first, int64_t n, void* me, void* psw, void* evw, cudaStream_t s);
 cudaError_t launch_fused_ggtt(const mg_process* p, uint64_t seed, uint64_t first, int64_t n, void* me, void* psw, void* evw, cudaStream_t s);

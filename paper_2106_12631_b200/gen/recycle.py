@@ -114,9 +114,10 @@ DEFAULTS = {
     2: dict(E=8, MINB=3, MINB32=3, EG=None, RELAXED='auto', SLOTS=0, BUDGET=240, HOIST=True, HPERM="2301", ORDER=None, FLIP=False),
     # FLIP (round 2): one warp (g g -> t t~ g g) / half a warp (g g -> t t~ g) per event, 16 / 32 events per SM.  Without it the
     # tuned shapes were E=4, MINB=4/5, HPERM="23104" and E=4, MINB=2/3, SLOTS=424, HPERM="320145", ORDER=(0, 3, 1, 2)
-    # (27.2 ms per 2^20 g g -> t t~ g g events against 17.5 ms; shapes timed: profiles/r02_h_*)
+    # (27.2 ms per 2^20 g g -> t t~ g g events against 17.1 ms; shapes and all 120 / 24 lane orders timed:
+    # profiles/r02_h_shapes_and_lane_orders.md)
     3: dict(E=8, MINB=4, MINB32=5, EG=None, RELAXED='auto', SLOTS=0, BUDGET=240, HOIST=True, HPERM="2310", ORDER=None, FLIP=True),
-    4: dict(E=8, MINB=2, MINB32=3, EG=None, RELAXED='auto', SLOTS=0, BUDGET=96, HOIST=True, HPERM="32014", ORDER=None, FLIP=True),
+    4: dict(E=8, MINB=2, MINB32=3, EG=None, RELAXED='auto', SLOTS=0, BUDGET=96, HOIST=True, HPERM="32410", ORDER=None, FLIP=True),
 }
 
 
@@ -528,8 +529,8 @@ def emit(prog):
     w("  static constexpr int NHEL_FULL = %d, NBITS = %d;" % (1 << npar, npar - (1 if prog.flip else 0)))
     w("  static constexpr int NMOM = %d, NSLOT = %d;" % (len(prog.mom_defs), prog.nslot))
     # lane bit i of a thread's index within its event carries the helicity of particle hperm[i]: t and t~ in the two
-    # lowest bits.  All 720 / 120 orders were timed on B200 with a run-time permutation, the best few rebuilt with the
-    # compile-time one: 2.7 % (g g -> t t~ g g) and 2 % (g g -> t t~ g) faster than particle order
+    # lowest bits.  Every order of the free particles was built and timed on B200 (profiles/r02_h_shapes_and_lane_orders.md):
+    # 17.1 .. 18.4 ms (g g -> t t~ g g), 4.39 .. 4.54 ms (g g -> t t~ g)
     hperm = prog.opts["HPERM"]
     assert sorted(hperm) == [str(i) for i in range(npar) if i != prog.fixed]
     w("  static constexpr unsigned HPERM = 0x%s;   // nibble i: particle whose helicity is bit i of the lane index" % hperm[::-1])
@@ -537,11 +538,10 @@ def emit(prog):
     w("  static __device__ __forceinline__ const rc::TermDesc& term(int i) { return kRcTerm_%s[i]; }" % tag)
     w("  static __device__ __forceinline__ rc::MomDef momdef(int i) { return kRcMom_%s[i]; }" % tag)
     w("")
-    w("  // producer steps, inner products, colour sum: |M|^2 of helicity h of event el (no g_s^(2 n_g)/denominator)")
-    w("  template <class T, class SM> static __device__ __forceinline__ T run(const SM& s, int tid, int el, int h, T mt) {")
+    w("  // producer steps and inner products (A6-A9): the colour-flow sums J_f of helicity h of event el")
+    w("  template <class T, class SM> static __device__ __forceinline__ void amplitudes(const SM& s, int tid, int el, int h, T mt, cx<T> (&jamp)[NFLOW]) {")
     w("    const typename SM::VW ev = s.view(el);")
     w("    const int grp = tid / NTG, gt = tid - grp * NTG, eb = grp * EG;   // synchronisation group, thread in it, its first event")
-    w("    cx<T> jamp[NFLOW];")
     seen = set()
     for si, (kind, items) in enumerate(prog.steps):
         if kind == "P":
@@ -604,7 +604,10 @@ def emit(prog):
                 w("    rc::sync_group<%s>(grp);" % name)
     assert len(seen) == nf
     num, den = prog.num, prog.den
-    w("    // A10: colour sum  sum_f C_ff |J_f|^2 + 2 sum_{f<g} C_fg Re(J_f^* J_g),  C = numerators / %d" % den)
+    w("  }")
+    w("")
+    w("  // A10: colour sum  sum_f C_ff |J_f|^2 + 2 sum_{f<g} C_fg Re(J_f^* J_g),  C = numerators / %d" % den)
+    w("  template <class T> static __device__ __forceinline__ T colour(const cx<T> (&jamp)[NFLOW]) {")
     w("    T me = (T)0;")
     for f in range(nf):
         w("    { T zr = (T)%d * jamp[%d].re, zi = (T)%d * jamp[%d].im;" % (num[f][f], f, num[f][f], f))
@@ -614,6 +617,13 @@ def emit(prog):
             w("      zr = fma_<T>((T)%d, jamp[%d].re, zr); zi = fma_<T>((T)%d, jamp[%d].im, zi);" % (2 * num[f][hh], hh, 2 * num[f][hh], hh))
         w("      me = fma_<T>(jamp[%d].re, zr, fma_<T>(jamp[%d].im, zi, me)); }" % (f, f))
     w("    return me * (T)%s;" % repr(1.0 / den))
+    w("  }")
+    w("")
+    w("  // |M|^2 of helicity h of event el (no g_s^(2 n_g)/denominator)")
+    w("  template <class T, class SM> static __device__ __forceinline__ T run(const SM& s, int tid, int el, int h, T mt) {")
+    w("    cx<T> jamp[NFLOW];")
+    w("    amplitudes<T, SM>(s, tid, el, h, mt, jamp);")
+    w("    return colour<T>(jamp);")
     w("  }")
     w("};")
     w("}  // namespace mg")

@@ -575,6 +575,45 @@ def test_host_form_chunked_path(mg, process, prec, n):
     assert P.last_kernel_ms() > 0
 
 
+@pytest.mark.parametrize("process,prec,n,chunk", [(2, 0, 5000 + 3, 1024), (2, 1, 4096, 0), (3, 0, 3000 + 5, 512), (3, 0, 2500, 0),
+                                                  (3, 1, 1500 + 1, 8), (3, 0, 7, 0)])
+def test_split_kernels_under_a_graph_give_the_same_values(mg, process, prec, n, chunk):
+    """mg_sigmakin_split (sigmaKin as smaller kernels under a CUDA graph): kernel A writes the
+    colour-flow sums, kernel B does colour and helicity sums; chunks alternate between two graph branches.  The arithmetic
+    is that of the single kernel, so the values are equal bit for bit (FP32: the single kernel without its double pass).
+    Ragged last chunk, n below one chunk, a second call that reuses the graph, a changed mask that rebuilds it."""
+    P = mg.Process(process, prec)
+    P.set_fp32_rescue(0.0)
+    ld = mg.padded_stride(n) + 32
+    mom = P.empty(4 * P.n_external, n, ld)
+    w = torch.empty(ld, dtype=P.dtype, device="cuda")
+    P.generate(7, 0, n, mom, w)
+    ew_ref = torch.zeros(ld, dtype=P.dtype, device="cuda")
+    ref = P.sigmakin(mom, n, ps_weight=w, event_weight=ew_ref)
+    me = torch.zeros(ld, dtype=P.dtype, device="cuda")
+    ew = torch.zeros(ld, dtype=P.dtype, device="cuda")
+    for _ in range(2):
+        me.zero_(); ew.zero_()
+        P.sigmakin_split(mom, n, me=me, ps_weight=w, event_weight=ew, chunk_events=chunk)
+        assert torch.equal(me[:n], ref[:n]) and torch.equal(ew[:n], ew_ref[:n])
+        assert (me[n:] == 0).all()
+    # oracle on a few events: the split path is compared with the paper's definition, not only with the other kernel
+    if prec == 0:
+        idx = torch.arange(0, n, max(1, n // 16))
+        aos = soa_to_aos(mom[:, idx].cpu().numpy().astype(np.float64), P.n_external)
+        assert np.abs(me[idx].cpu().numpy() / oracle.me(process, aos) - 1).max() < 1e-12
+    full = P.helicity_mask()
+    P.set_helicity_mask(full & 0x5555555555555555)
+    ref2 = P.sigmakin(mom, n)
+    P.sigmakin_split(mom, n, me=me, chunk_events=chunk)
+    assert torch.equal(me[:n], ref2[:n]) and not torch.equal(ref2[:n], ref[:n])
+    P.set_helicity_mask(full)
+    with pytest.raises(mg.MgError):
+        P.sigmakin_split(mom, n, me=me, chunk_events=12)
+    with pytest.raises(mg.MgError):
+        mg.Process(1, 0).sigmakin_split(mom, n, me=me)
+
+
 def test_sharded_sums_on_one_device(mg):
     """shard.gpu_compute (the compute leg of the multi-GPU path) on one device: world 1 and two
     emulated ranks (rank/world passed explicitly) merge to the same sums, which match the oracle on the same events."""
