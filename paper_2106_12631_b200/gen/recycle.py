@@ -116,7 +116,9 @@ DEFAULTS = {
     # tuned shapes were E=4, MINB=4/5, HPERM="23104" and E=4, MINB=2/3, SLOTS=424, HPERM="320145", ORDER=(0, 3, 1, 2)
     # (27.2 ms per 2^20 g g -> t t~ g g events against 17.1 ms; shapes and all 120 / 24 lane orders timed:
     # profiles/r02_h_shapes_and_lane_orders.md)
-    3: dict(E=8, MINB=4, MINB32=5, EG=None, RELAXED='auto', SLOTS=0, BUDGET=240, HOIST=True, HPERM="2310", ORDER=None, FLIP=True),
+    # g g -> t t~ g: 96 entries in 6 steps instead of 112 in 4 (BUDGET) so that 32 instead of 24 events fit an SM in FP64, as 2 CTAs
+    # of 16 events: 4.39 -> 3.71 ms per 2^21 events (FP32, 4 CTAs: 2.59 -> 2.35); profiles/r02_h_shapes_and_lane_orders.md
+    3: dict(E=16, MINB=2, MINB32=4, EG=None, RELAXED='auto', SLOTS=0, BUDGET=64, HOIST=True, HPERM="2310", ORDER=None, FLIP=True),
     4: dict(E=8, MINB=2, MINB32=3, EG=None, RELAXED='auto', SLOTS=0, BUDGET=96, HOIST=True, HPERM="32410", ORDER=None, FLIP=True),
 }
 
