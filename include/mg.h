@@ -50,7 +50,7 @@ typedef struct mg_process mg_process; /* opaque; owns constant tables, two strea
 
 enum { MG_EEMUMU = 0, MG_GGTT = 1, MG_GGTTG = 2, MG_GGTTGG = 3, MG_QQTT = 4, MG_QQTTG = 5 };
 enum { MG_FP64 = 0, MG_FP32 = 1 };
-enum { MG_OK = 0, MG_EINVAL = -1, MG_EPARAM = -2, MG_ECUDA = -3, MG_ENOMEM = -4 };
+enum { MG_OK = 0, MG_EINVAL = -1, MG_EPARAM = -2, MG_ECUDA = -3, MG_ENOMEM = -4, MG_ELIMIT = -5 };
 /* stages for mg_flops_per_event / mg_bytes_per_event */
 enum { MG_STAGE_RNG = 0, MG_STAGE_RAMBO = 1, MG_STAGE_SIGMAKIN = 2, MG_STAGE_GENERATE = 3 };
 
@@ -160,6 +160,24 @@ int mg_unweight(mg_process* p, uint64_t seed, uint64_t first_event, const void* 
 int mg_weight_sums_async(mg_process* p, const void* d_weights, int64_t n, double* d_sums_out, void* stream);
 int mg_unweight_async(mg_process* p, uint64_t seed, uint64_t first_event, const void* d_weights, int64_t n, double w_max,
                       int64_t* d_kept_out, int64_t* d_count_out, void* stream);
+
+/* mg_weight_sums_async WITHOUT any allocation, for callers that may not call cudaMalloc (code under CUDA graph
+ * capture, tight serving loops, harnesses that forbid it): d_sums_out[0..2] = (sum w, sum w^2, max w) over the n event
+ * weights d_weights[n], the same kernels, the same order of additions and therefore the same bits as
+ * mg_weight_sums_async.  The per-CTA partial sums between its two kernels live in a
+ * fixed 48 KB array in the library's device image (csrc/xsec.cu) instead of the handle's scratch region, which
+ * cudaMalloc grows on demand; every GPU that loads the library holds that array until the process exits.
+ *  - Limit: n <= mg_weight_sums_static_max_events() = 2^24 (the largest batch of BASELINE.json); MG_ELIMIT beyond it.
+ *  - Allocates nothing and frees nothing, on the host or the device.  The first call on a device asks the runtime for
+ *    the array's device address (a lookup, not an allocation); make that first call outside a stream capture.
+ *  - All calls on a device share the array (all handles, all streams) and there is NO ordering between them: calls
+ *    that overlap on the GPU — different streams, or graphs launched concurrently — race on it; keep them on one
+ *    stream or order them with events.  Nothing in the array has to start at zero (the second kernel reads only the
+ *    partials the first kernel of the same call has written); what a call leaves behind is never read.
+ * Asynchronous on `stream`; results stay on the device.  n == 0 writes three zeros.
+ * Errors: MG_EINVAL (NULL or misaligned pointer, n < 0, bad handle), MG_ELIMIT, MG_ECUDA. */
+int mg_weight_sums_static(mg_process* p, const void* d_weights, int64_t n, double* d_sums_out, void* stream);
+int64_t mg_weight_sums_static_max_events(void);
 
 /* A12: good-helicity filter (R16).  Evaluates every helicity combination on the
  * first probe_n events of d_momenta (1 <= probe_n <= n... the caller guarantees probe_n events are

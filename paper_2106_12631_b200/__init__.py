@@ -71,6 +71,8 @@ def lib():
         "mg_bytes_per_event": (i64, [vp, C.c_int]),
         "mg_last_kernel_ms": (C.c_double, [vp]),
         "mg_weight_sums_async": (C.c_int, [vp, vp, i64, vp, vp]),
+        "mg_weight_sums_static": (C.c_int, [vp, vp, i64, vp, vp]),
+        "mg_weight_sums_static_max_events": (i64, []),
         "mg_unweight_async": (C.c_int, [vp, u64, u64, vp, i64, C.c_double, vp, vp, vp]),
         "mg_set_fp32_rescue": (C.c_int, [vp, C.c_double]),
         "mg_get_fp32_rescue": (C.c_double, [vp]),
@@ -90,7 +92,7 @@ EXPORTED = ["mg_default_params", "mg_init_process", "mg_free_process", "mg_n_ext
             "mg_padded_stride", "mg_rng_words", "mg_rng", "mg_rambo", "mg_generate", "mg_filter_helicities",
             "mg_set_helicity_mask", "mg_get_helicity_mask", "mg_sigmakin", "mg_sigmakin_per_helicity", "mg_sigmakin_fused", "mg_sigmakin_split", "mg_weight_sums", "mg_unweight",
             "mg_sigmakin_host", "mg_run_host", "mg_flops_per_event", "mg_bytes_per_event", "mg_last_kernel_ms",
-            "mg_weight_sums_async", "mg_unweight_async", "mg_set_fp32_rescue", "mg_get_fp32_rescue", "mg_last_rescued",
+            "mg_weight_sums_async", "mg_unweight_async", "mg_weight_sums_static", "mg_weight_sums_static_max_events", "mg_set_fp32_rescue", "mg_get_fp32_rescue", "mg_last_rescued",
             "mg_strerror", "mg_version"]
 
 
@@ -101,6 +103,11 @@ def _check(rc):
 
 def padded_stride(n):
     return int(lib().mg_padded_stride(n))
+
+
+def weight_sums_static_max_events():
+    """Largest n mg_weight_sums_static accepts (its partial sums live in a fixed device array of the library)."""
+    return int(lib().mg_weight_sums_static_max_events())
 
 
 def default_params(process, precision=FP64, device=0, **kw):
@@ -240,6 +247,12 @@ class Process:
         """mg_weight_sums_async: (sum w, sum w^2, max w) left on the device (float64[3]); no host synchronisation."""
         out = out if out is not None else torch.empty(3, dtype=torch.float64, device=self.device)
         _check(lib().mg_weight_sums_async(self._h, _ptr(weights), n, _ptr(out), _stream(self.device)))
+        return out
+
+    def weight_sums_static(self, weights, n, out):
+        """mg_weight_sums_static: mg_weight_sums_async with its partial sums in a fixed device array of the library: no
+        allocation anywhere (`out`, float64[3] on the device, is the caller's); n <= weight_sums_static_max_events()."""
+        _check(lib().mg_weight_sums_static(self._h, _ptr(weights), n, _ptr(out), _stream(self.device)))
         return out
 
     def unweight_async(self, seed, first_event, weights, n, w_max, kept=None, count=None):

@@ -605,6 +605,7 @@ const char* mg_strerror(int code) {
     case MG_EPARAM: return "unphysical parameters";
     case MG_ECUDA: return "CUDA error or no sm_100 device";
     case MG_ENOMEM: return "out of memory";
+    case MG_ELIMIT: return "size above the fixed maximum of a no-allocation entry point (mg_weight_sums_static_max_events)";
   }
   return "unknown error";
 }

@@ -146,6 +146,35 @@ cudaError_t launch_weight_sums(const mg_process* p, const void* d_w, int64_t n, 
   return cudaGetLastError();
 }
 
+// ---------------------------------------------------------------------------------------------------
+// mg_weight_sums_static: the weight sums WITHOUT any allocation (include/mg.h).  The per-CTA partials of pass 1 live in a
+// file-scope device array instead of the handle's scratch region (which cudaMalloc grows on demand): for callers that
+// may not allocate — code under CUDA graph capture, tight serving loops, harnesses that forbid cudaMalloc.
+// Limit: kStaticMaxEvents events per call (the largest batch of BASELINE.json); the array is 48 KB and every GPU that
+// loads the library holds it until the process exits.  All calls on a device share it; pass 2 reads only partials
+// that pass 1 of the SAME call has written, so nothing in it has to start at zero and the contents the previous call
+// left behind are never read — but two calls that overlap on the GPU (different streams) race on it.
+// ---------------------------------------------------------------------------------------------------
+constexpr int64_t kStaticMaxEvents = (int64_t)1 << 24;
+constexpr int64_t kStaticMaxBlocks = kStaticMaxEvents / ((int64_t)kTile * kItems);      // 2048 CTAs
+static __device__ __align__(256) double g_ws_static_partials[3 * kStaticMaxBlocks];     // 49 152 bytes
+
+// In host code the array's name is only a stand-in: its device address is asked for once per device, with that
+// device current (not an allocation: the array is part of the loaded module)
+static cudaError_t static_partials(int device, double** out) {
+  static double* addr[64];
+  if (device < 0 || device >= 64) return cudaErrorInvalidDevice;
+  if (addr[device] == nullptr) {
+    double* q = nullptr;
+    const cudaError_t e = cudaGetSymbolAddress((void**)&q, g_ws_static_partials);
+    if (e != cudaSuccess) return e;
+    if (q == nullptr) return cudaErrorInvalidSymbol;
+    addr[device] = q;
+  }
+  *out = addr[device];
+  return cudaSuccess;
+}
+
 int64_t unweight_tiles(int64_t n) { return (n + kUwTile - 1) / kUwTile; }
 
 cudaError_t launch_unweight(const mg_process* p, uint64_t seed, uint64_t first, const void* d_w, int64_t n, double wmax,
@@ -161,3 +190,31 @@ cudaError_t launch_unweight(const mg_process* p, uint64_t seed, uint64_t first, 
 }
 
 }  // namespace mg
+
+extern "C" {
+
+int64_t mg_weight_sums_static_max_events(void) { return mg::kStaticMaxEvents; }
+
+int mg_weight_sums_static(mg_process* p, const void* d_weights, int64_t n, double* d_sums_out, void* stream) {
+  if (p == nullptr || n < 0 || d_sums_out == nullptr || ((uintptr_t)d_sums_out % sizeof(double)) != 0) return MG_EINVAL;
+  if (n > mg::kStaticMaxEvents) return MG_ELIMIT;
+  const size_t es = p->par.precision == MG_FP64 ? 8 : 4;
+  if (n > 0 && (d_weights == nullptr || ((uintptr_t)d_weights % es) != 0)) return MG_EINVAL;
+  int prev = -1;
+  if (cudaGetDevice(&prev) != cudaSuccess) { cudaGetLastError(); return MG_ECUDA; }
+  if (prev != p->par.device && cudaSetDevice(p->par.device) != cudaSuccess) { cudaGetLastError(); return MG_ECUDA; }
+  cudaStream_t s = (cudaStream_t)stream;
+  cudaError_t e;
+  if (n == 0) {
+    e = cudaMemsetAsync(d_sums_out, 0, 3 * sizeof(double), s);
+  } else {
+    double* d_part = nullptr;
+    e = mg::static_partials(p->par.device, &d_part);
+    if (e == cudaSuccess) e = mg::launch_weight_sums(p, d_weights, n, d_part, d_sums_out, s);
+  }
+  if (e != cudaSuccess) cudaGetLastError();
+  if (prev != p->par.device) cudaSetDevice(prev);
+  return e == cudaSuccess ? MG_OK : MG_ECUDA;
+}
+
+}  // extern "C"
