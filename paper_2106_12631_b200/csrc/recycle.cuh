@@ -29,7 +29,9 @@
 namespace mg {
 namespace rc {
 
-enum Kind { K_POLVEC = 0, K_UBAR = 1, K_VSP = 2, K_VCUR = 3, K_ROWPROP = 4, K_COLPROP = 5, K_FFCUR = 6, K_SLASHCOL = 7, K_SLASHROW = 8, K_EXT = 9 };
+enum Kind { K_POLVEC = 0, K_UBAR = 1, K_VSP = 2, K_VCUR = 3, K_ROWPROP = 4, K_COLPROP = 5, K_FFCUR = 6, K_SLASHCOL = 7, K_SLASHROW = 8, K_EXT = 9,
+            // the same four operations on a signed SUM of slash products (terms in the term table; gen/recycle.py _presum)
+            K_ROWPROPN = 10, K_COLPROPN = 11, K_SLASHCOLN = 12, K_SLASHROWN = 13 };
 
 // operand word: low 16 bits = first entry of the operand node, high 16 bits = 4 * mask, where mask says which of
 // the consumer's variant bits select the operand's variant (pext through the per-variant table, see pext4)
@@ -42,7 +44,8 @@ struct NodeDesc {
   int nterm;        // K_VCUR: number of terms
   Op op[2];
 };
-struct TermDesc {   // one term of a gluon current: type 0: V3(A,kA,B,kB);  1..3: four-gluon structure `type`(A,B,C)
+struct TermDesc {   // one term of a gluon current: type 0: V3(A,kA,B,kB);  1..3: four-gluon structure `type`(A,B,C);
+                    // one term of a sum of slash products (K_*N nodes): op[0] = spinor, op[1] = vector, signbit
   short type;
   short momA, momB, pad;
   unsigned int signbit;   // 0 or 0x80000000: the term enters with sign -1
@@ -215,6 +218,28 @@ MG_RC_TASK(K_SLASHROW) {  // half product psibar Vslash (op0 = psibar, op1 = V)
   const Vec4<T> V = ev.ldv(entry_of(d.op[1], pt));
   ev.sts(d.out + v, slash_row(slash_parts(V), s));
 } };
+// sum_i (+-) psibar_i Vslash_i (ROW) or sum_i (+-) Vslash_i psi_i: wavefunctions that enter the same colour-flow sums with the
+// same partner are added up before the propagator / before the inner product (linearity; gen/recycle.py _presum)
+template <class P, class T, bool ROW, class VW> __device__ __forceinline__ Spinor<T> slash_sum(const NodeDesc& d, unsigned long long pt, const VW& ev) {
+  Spinor<T> acc;
+  for (int it = 0; it < d.nterm; ++it) {
+    const TermDesc& t = P::term(d.aux + it);
+    const Spinor<T> s = ev.lds(entry_of(t.op[0], pt));
+    const Vec4<T> V = ev.ldv(entry_of(t.op[1], pt));
+    const Spinor<T> x = ROW ? slash_row(slash_parts(V), s) : slash_col(slash_parts(V), s);
+    if (it == 0) {
+      acc.l[0] = flip(x.l[0], t.signbit); acc.l[1] = flip(x.l[1], t.signbit); acc.r[0] = flip(x.r[0], t.signbit); acc.r[1] = flip(x.r[1], t.signbit);
+    } else {
+      acc.l[0] = acc.l[0] + flip(x.l[0], t.signbit); acc.l[1] = acc.l[1] + flip(x.l[1], t.signbit);
+      acc.r[0] = acc.r[0] + flip(x.r[0], t.signbit); acc.r[1] = acc.r[1] + flip(x.r[1], t.signbit);
+    }
+  }
+  return acc;
+}
+MG_RC_TASK(K_ROWPROPN) { ev.sts(d.out + v, scale(ev.ip[d.prop], qslash_m_row(ev.ldm(d.mom), mt, slash_sum<P, T, true>(d, pt, ev)))); } };
+MG_RC_TASK(K_COLPROPN) { ev.sts(d.out + v, scale(ev.ip[d.prop], qslash_m_col(ev.ldm(d.mom), mt, slash_sum<P, T, false>(d, pt, ev)))); } };
+MG_RC_TASK(K_SLASHCOLN) { ev.sts(d.out + v, slash_sum<P, T, false>(d, pt, ev)); } };
+MG_RC_TASK(K_SLASHROWN) { ev.sts(d.out + v, slash_sum<P, T, true>(d, pt, ev)); } };
 #undef MG_RC_TASK
 
 // shared memory of one CTA

@@ -22,7 +22,7 @@ import os
 from collections import OrderedDict
 
 from . import qcdgen
-from .qcdgen import (F_FF_CUR, F_FFV_PROP, F_MDOT_VV, F_POLVEC, F_ROW_COL, F_SCALE, F_SLASH, F_SLASH_PARTS,
+from .qcdgen import (F_FF_CUR, F_FFV_PROP, F_MDOT_VV, F_POLVEC, F_QSLASH, F_ROW_COL, F_SCALE, F_SLASH, F_SLASH_PARTS,
                      F_SPINOR, F_VVV_CUR, F_VVVV_CUR)
 
 CSRC = qcdgen.CSRC
@@ -59,7 +59,7 @@ class RNode:
         return 1 << len(self.dep)
 
     def operands(self):
-        if self.kind == "VCUR":
+        if "terms" in self.params:
             out = []
             for t in self.params["terms"]:
                 out.extend(t["ops"])
@@ -84,6 +84,9 @@ class RNode:
             return F_FFV_PROP
         if k == "FFCUR":
             return F_FF_CUR + F_SCALE
+        if k in ("ROWPROPN", "COLPROPN", "SLASHCOLN", "SLASHROWN"):      # sum of slash products, then at most one propagator
+            nt = len(self.params["terms"])
+            return nt * (F_SLASH_PARTS + F_SLASH) + 8 * (nt - 1) + (F_QSLASH + F_SCALE if k.endswith("PROPN") else 0)
         return F_SLASH_PARTS + F_SLASH
 
 
@@ -108,18 +111,20 @@ def _closure_key(c):
 #   HPERM             lane bit i of a thread's index within its event carries the helicity of particle HPERM[i]
 #   FLIP              helicity-flip symmetry (R35): the last particle's helicity is fixed at -1, one thread per
 #                     combination of the OTHER helicities; |M|^2 counts for the combination and its complement
+#   PRESUM            wavefunctions that enter the same colour-flow sums with the same partner are added up BEFORE the
+#                     inner product: sum_i s_i (R_i . C) = (sum_i s_i R_i) . C, rows first, then columns (_presum)
 #   ORDER             order of the closure classes (indices into the classes sorted by (helicity bits, kind) of their
 #                     half product); None = sorted
 DEFAULTS = {
-    2: dict(E=8, MINB=3, MINB32=3, EG=None, RELAXED='auto', SLOTS=0, BUDGET=240, HOIST=True, HPERM="2301", ORDER=None, FLIP=False),
+    2: dict(E=8, MINB=3, MINB32=3, EG=None, RELAXED='auto', SLOTS=0, BUDGET=240, HOIST=True, HPERM="2301", ORDER=None, FLIP=False, PRESUM=False),
     # FLIP (round 2): one warp (g g -> t t~ g g) / half a warp (g g -> t t~ g) per event, 16 / 32 events per SM.  Without it the
     # tuned shapes were E=4, MINB=4/5, HPERM="23104" and E=4, MINB=2/3, SLOTS=424, HPERM="320145", ORDER=(0, 3, 1, 2)
     # (27.2 ms per 2^20 g g -> t t~ g g events against 17.1 ms; shapes and all 120 / 24 lane orders timed:
     # profiles/r02_h_shapes_and_lane_orders.md)
     # g g -> t t~ g: 96 entries in 6 steps instead of 112 in 4 (BUDGET) so that 32 instead of 24 events fit an SM in FP64, as 2 CTAs
     # of 16 events: 4.39 -> 3.71 ms per 2^21 events (FP32, 4 CTAs: 2.59 -> 2.35); profiles/r02_h_shapes_and_lane_orders.md
-    3: dict(E=16, MINB=2, MINB32=4, EG=None, RELAXED='auto', SLOTS=0, BUDGET=64, HOIST=True, HPERM="2310", ORDER=None, FLIP=True),
-    4: dict(E=8, MINB=2, MINB32=3, EG=None, RELAXED='auto', SLOTS=0, BUDGET=96, HOIST=True, HPERM="32410", ORDER=None, FLIP=True),
+    3: dict(E=16, MINB=2, MINB32=4, EG=None, RELAXED='auto', SLOTS=0, BUDGET=64, HOIST=True, HPERM="2310", ORDER=None, FLIP=True, PRESUM=False),
+    4: dict(E=8, MINB=2, MINB32=3, EG=None, RELAXED='auto', SLOTS=0, BUDGET=96, HOIST=True, HPERM="32410", ORDER=None, FLIP=True, PRESUM=True),
 }
 
 
@@ -146,6 +151,8 @@ class Program:
         self._build_momenta()
         self._build_nodes()
         self._build_closures()
+        if o["PRESUM"]:
+            self._presum()
         self._schedule(o["BUDGET"])
         if self.RELAXED == 'auto':
             self.RELAXED = '0'
@@ -264,6 +271,87 @@ class Program:
                 nfull += 1
                 self.half[key] = self._vcur(key, frozenset(range(self.ng)), terms, prop=None)
                 self.closures.append(Closure("DOTV", self.half[key], self.nodes["G"], flows))
+
+    # ------------------------------------------------------------------ pre-summed closures
+    def _presum(self):
+        """The closures add x_c = a_c . b_c into the colour-flow sums, J_f += sum_c s_fc x_c.  For the closures that share
+        the operand b, J_f += (sum_a s_f,a a) . b: one inner product per DISTINCT signed sum of rows among the flows instead
+        of one per row, and one update per (sum, flow) instead of one per (row, flow).  Applied to the rows of every b, then
+        to the columns of every (summed) row, wherever it lowers the number of inner products: for a quark line with two
+        gluons on either side of the cut this turns 9 products and 16 updates into 4 and 4 — the colour-ordered sub-currents
+        found from the sign tables alone.  A sum is a task like any other (kind SUM: signed sum of stored wavefunctions),
+        computed once per event and helicity variant."""
+        cl = [(c.a, c.b, OrderedDict(c.flows), c.kind) for c in self.closures]
+        sums = OrderedDict()
+        for side in (0, 1):
+            groups = OrderedDict()
+            for a, b, fl, kind in cl:
+                key, x = (b, a) if side == 0 else (a, b)
+                groups.setdefault(key.name, (key, kind, []))[2].append((x, fl))
+            out = []
+            for key, kind, items in groups.values():
+                byname = dict((x.name, x) for x, _ in items)
+                per_flow = OrderedDict()
+                for x, fl in items:
+                    for fidx, sg in fl.items():
+                        u = per_flow.setdefault(fidx, OrderedDict())
+                        u[x.name] = u.get(x.name, 0) + sg
+                distinct = OrderedDict()
+                for fidx in sorted(per_flow):
+                    u = dict((n, sg) for n, sg in per_flow[fidx].items() if sg)
+                    assert u and all(abs(sg) == 1 for sg in u.values())
+                    lead = 1 if u[min(u)] > 0 else -1
+                    distinct.setdefault(tuple(sorted((n, sg * lead) for n, sg in u.items())), OrderedDict())[fidx] = lead
+                if kind != "DOTS" or len(distinct) >= len(items):     # all-gluon closures: their sums would need every J alive at once
+                    for x, fl in items:
+                        out.append((x, key, fl, kind) if side == 0 else (key, x, fl, kind))
+                    continue
+                for combo, fl in distinct.items():
+                    if len(combo) == 1:
+                        x = byname[combo[0][0]]
+                        fl = OrderedDict((fidx, lead * combo[0][1]) for fidx, lead in fl.items())
+                    else:
+                        if combo not in sums:
+                            ops = [byname[n] for n, _ in combo]
+                            dep = set()
+                            for o in ops:
+                                dep |= set(o.dep)
+                            sums[combo] = RNode("S%d_%d" % (side, len(sums)), "SUM", dep, ops, signs=[sg for _, sg in combo])
+                        x = sums[combo]
+                    out.append((x, key, fl, kind) if side == 0 else (key, x, fl, kind))
+            cl = out
+        # A sum is not stored as a sum of stored wavefunctions: the operation that made its operands is linear, so the sum
+        # is ONE task of the same kind with several (spinor, vector, sign) terms — psibar' = [sum_i s_i psibar_i Vslash_i]
+        # (qslash + m)/(q^2 - m^2) for rows that share their line momentum, sum_i s_i Vslash_i psi_i for half products —
+        # and the operands themselves are dropped where nothing else reads them
+        fused_kind = {"ROWPROP": "ROWPROPN", "COLPROP": "COLPROPN", "SLASHCOL": "SLASHCOLN", "SLASHROW": "SLASHROWN"}
+        repl = {}
+        for node in sums.values():
+            kinds = set(o.kind for o in node.ops)
+            assert len(kinds) == 1 and kinds <= set(fused_kind), (node.name, kinds)
+            k0 = node.ops[0].kind
+            par = dict(terms=[dict(type=0, sign=sg, ops=[o.ops[0], o.ops[1]], momA=0, momB=0) for o, sg in zip(node.ops, node.params["signs"])])
+            if k0 in ("ROWPROP", "COLPROP"):
+                assert len(set((o.params["mom"], o.params["prop"]) for o in node.ops)) == 1, node.name
+                par.update(mom=node.ops[0].params["mom"], prop=node.ops[0].params["prop"])
+            repl[node.name] = RNode(node.name + "_" + "_".join(o.name for o in node.ops), fused_kind[k0], node.dep, [], **par)
+            if k0 in ("SLASHCOL", "SLASHROW"):
+                self.half[repl[node.name].name] = repl[node.name]
+            else:
+                self.nodes[repl[node.name].name] = repl[node.name]
+        cl = [(repl.get(a.name, a), repl.get(b.name, b), fl, kind) for a, b, fl, kind in cl]
+        used = set()
+        for a, b, fl, kind in cl:
+            used.update((a.name, b.name))
+        for n in list(self.nodes.values()) + list(self.half.values()):
+            used.update(o.name for o in n.operands())
+        for name in [x for x in self.half if x not in used]:
+            del self.half[name]
+        for name in [x for x in self.nodes if x not in used]:
+            del self.nodes[name]
+        self.closures = [Closure(kind, a, b, list(fl.items())) for a, b, fl, kind in cl]
+        for c in self.closures:
+            assert (c.a.name in self.half) != (c.b.name in self.half), (c.a.name, c.b.name)
 
     # ------------------------------------------------------------------ steps
     def _schedule(self, budget):
@@ -497,7 +585,7 @@ def emit(prog):
     for n in order:
         ops = ["0u", "0u"]
         aux, nterm = 0, 0
-        if n.kind == "VCUR":
+        if "terms" in n.params:            # VCUR; sums of slash products (type 0: op0 = spinor, op1 = vector)
             aux, nterm = len(terms), len(n.params["terms"])
             for t in n.params["terms"]:
                 tops = t["ops"] if t["type"] == 0 else t["cops"]

@@ -147,6 +147,13 @@ def run(prog, mom, mt, gs):
                         r = ip[n.params["prop"]] * (slash_col(q, slash_col(get(n.ops[1], v, n), get(n.ops[0], v, n))) + mt * slash_col(get(n.ops[1], v, n), get(n.ops[0], v, n)))
                     elif n.kind == "FFCUR":
                         r = ip[n.params["prop"]] * ff_current(get(n.ops[0], v, n), get(n.ops[1], v, n))
+                    elif n.kind in ("ROWPROPN", "COLPROPN", "SLASHCOLN", "SLASHROWN"):
+                        # the same operations on a signed sum of slash products (gen/recycle.py _presum)
+                        sl = slash_row if n.kind in ("ROWPROPN", "SLASHROWN") else slash_col
+                        r = sum(t["sign"] * sl(get(t["ops"][1], v, n), get(t["ops"][0], v, n)) for t in n.params["terms"])
+                        if n.kind.endswith("PROPN"):
+                            q = tab[n.params["mom"]]
+                            r = ip[n.params["prop"]] * (sl(q, r) + mt * r)
                     elif n.kind == "SLASHCOL":
                         r = slash_col(get(n.ops[1], v, n), get(n.ops[0], v, n))
                     elif n.kind == "SLASHROW":

@@ -62,8 +62,12 @@ def test_program_is_the_same_function_of_momenta_rounded_to_fp32(programs, ng, n
 
 def test_program_shape(programs):
     # one closure per colour-ordered amplitude of the diagram list: 3 / 18 / 159 amplitudes collapse to
-    # 3 / 15 / 105 inner products once diagrams that differ only in a gluon sub-tree share an off-shell current
-    assert [len(programs[ng].closures) for ng in (2, 3, 4)] == [3, 15, 105]
+    # 3 / 15 / 105 inner products once diagrams that differ only in a gluon sub-tree share an off-shell current;
+    # g g -> t t~ g g: 75 after the rows and columns that enter the same colour-flow sums are added up before the
+    # product (PRESUM: the six classes with two gluons on either side of the cut go from 9 products and 16 updates to 4 and 4)
+    assert [len(programs[ng].closures) for ng in (2, 3, 4)] == [3, 15, 75]
+    assert len(recycle.Program(4, PRESUM=False).closures) == 105
+    assert sum(len(c.flows) for c in programs[4].closures) == 264 and sum(len(c.flows) for c in recycle.Program(4, PRESUM=False).closures) == 336
     for ng, prog in programs.items():
         assert prog.nhel == 1 << (ng + 2 - (1 if prog.flip else 0))       # threads per event (FLIP: the last helicity is fixed)
         # every node is written before it is read and its slots lie inside the allocated entries
