@@ -21,15 +21,17 @@ struct Eemumu {
   static constexpr int NHEL = 16;
   static constexpr int NPAR = 4;
   static constexpr bool FLIP = false;   // chiral Z couplings: |M(h)|^2 != |M(-h)|^2
-#ifndef MG_EE_MINB
-#define MG_EE_MINB 6
-#endif
-  static constexpr int MINB = MG_EE_MINB;   // resident CTAs of 128 threads the register allocation aims at
+  // resident CTAs of 128 threads the register allocation aims at (measured on B200, 2^24 events): FP32 6 (64 registers, no
+  // spills: 0.408 ms); FP64 holds the four currents in 64 registers: 5 CTAs (96 registers) 0.735 ms, 4 (122) 0.756, 6 (80) 0.872
+  static constexpr int MINB = 6, MINB64 = 5;
   // Massless helicity spinors need three reals per particle (the "simplified" IXXXXX/OXXXXX of PAPER.md:136):
   //   omega_+ chi_+ = (a, b),  omega_+ chi_- = (-b^*, a),   a = sqrt(P+pz),  b = (px + i py)/sqrt(P+pz),
   // P+pz evaluated as pT^2/(P-pz) for pz < 0 (R19); along -z: a = 0, b = sqrt(2P) (B1).  One square root, one
   // reciprocal square root and at most one division per particle and event, shared by all 16 helicity combinations.
-  template <class T> struct Event { Mom<T> p[4]; Mom<T> q; T is; cx<T> bw; T a[4]; cx<T> b[4]; };
+  // Each of the two currents has ONE non-zero helicity assignment per chirality, so all 16 helicity combinations share
+  // four currents and their four contractions with q: they are evaluated once per event (finish), and a helicity
+  // combination only selects one of each and does the final contraction (helicity)
+  template <class T> struct Event { Mom<T> p[4]; Mom<T> q; T is; cx<T> bw; Vec4<T> JeR, JeL, JmR, JmL; cx<T> qeR, qeL, qmR, qmL; };
 
   template <class T> static MG_HD void massless_frame(Mom<T> p, T& a, cx<T>& b) {
     const T px = p.v[1], py = p.v[2], pz = p.v[3];
@@ -54,8 +56,19 @@ struct Eemumu {
     const T dr = s - (T)k.mZ2, di = (T)k.mZgZ;
     const T inv = (T)1 / fma_<T>(dr, dr, di * di);
     ev.bw = cx<T>(dr * inv, -di * inv);
-#pragma unroll
-    for (int i = 0; i < 4; ++i) massless_frame<T>(ev.p[i], ev.a[i], ev.b[i]);
+    T a0, a1, a2, a3;
+    cx<T> b0, b1, b2, b3;
+    massless_frame<T>(ev.p[0], a0, b0); massless_frame<T>(ev.p[1], a1, b1);
+    massless_frame<T>(ev.p[2], a2, b2); massless_frame<T>(ev.p[3], a3, b3);
+    // the e+ e- current and the mu+ mu- current vanish unless the two helicities of a line are opposite, and each is a
+    // single chirality block:
+    //   vbar(e+, h0) gamma^mu u(e-, h1):   h1 = +1: a = (-a0, -b0^*), psi_R = (a1, b1)       h1 = -1: b = (-b0, a0), psi_L = (-b1^*, a1)
+    //   ubar(mu-, h3) gamma^mu v(mu+, h2): h3 = +1: a = (a3, b3^*),  psi_R = (-a2, -b2)      h3 = -1: b = (-b3, a3), psi_L = (-b2^*, a2)
+    ev.JeR = cur_R<T>(cx<T>(-a0, (T)0), -conj_(b0), cx<T>(a1, (T)0), b1);
+    ev.JeL = cur_L<T>(-b0, cx<T>(a0, (T)0), -conj_(b1), cx<T>(a1, (T)0));
+    ev.JmR = cur_R<T>(cx<T>(a3, (T)0), conj_(b3), cx<T>(-a2, (T)0), -b2);
+    ev.JmL = cur_L<T>(-b3, cx<T>(a3, (T)0), -conj_(b2), cx<T>(a2, (T)0));
+    ev.qeR = mdot(ev.JeR, ev.q); ev.qeL = mdot(ev.JeL, ev.q); ev.qmR = mdot(ev.JmR, ev.q); ev.qmL = mdot(ev.JmL, ev.q);
   }
 
   // psibar gamma^mu psi of a massless line: only one chirality block of each spinor is non-zero, so the current is ONE of
@@ -74,27 +87,23 @@ struct Eemumu {
   }
 
   // |M|^2 of one helicity combination.  The helicity index is the same for every thread of the launch (the loop over the
-  // good-helicity mask is uniform), so the chirality cases below are uniform branches, not divergence.
-  // Massless leptons: the e+ e- current and the mu+ mu- current vanish unless the two helicities of a line are opposite,
-  // and each is a single chirality block:
-  //   vbar(e+, h0) gamma^mu u(e-, h1):   h1 = +1: a = (-a0, -b0^*), psi_R = (a1, b1)       h1 = -1: b = (-b0, a0), psi_L = (-b1^*, a1)
-  //   ubar(mu-, h3) gamma^mu v(mu+, h2): h3 = +1: a = (a3, b3^*),  psi_R = (-a2, -b2)      h3 = -1: b = (-b3, a3), psi_L = (-b2^*, a2)
-  // (the table above, written out).  With J_e, J_m and the chiral Z couplings g_e, g_m of the two blocks:
+  // good-helicity mask is uniform), so the selections below are uniform, not divergence.  With the
+  // currents J_e, J_m of the combination and the chiral Z couplings g_e, g_m of their blocks:
   //   FFV1P0_3 + FFV1_0 :   amp_a = e^2 (J_e . J_m) / s
   //   FFV2_4_3 + FFV2_4_0:  amp_b = g_e g_m [ (J_e . J_m) - (J_e . q)(J_m . q)/mZ^2 ] / (s - mZ^2 + i mZ GZ)      (R13)
   template <class T> static MG_HD T helicity(const Event<T>& ev, int ihel, const Consts& k) {
     const bool h0 = (ihel & 1) != 0, h1 = (ihel & 2) != 0, h2 = (ihel & 4) != 0, h3 = (ihel & 8) != 0;
     if (h0 == h1 || h2 == h3) return (T)0;
-    const T a0 = ev.a[0], a1 = ev.a[1], a2 = ev.a[2], a3 = ev.a[3];
-    const cx<T> b0 = ev.b[0], b1 = ev.b[1], b2 = ev.b[2], b3 = ev.b[3];
-    Vec4<T> Je, Jm;
-    T ge, gm;
-    if (h1) { Je = cur_R<T>(cx<T>(-a0, (T)0), -conj_(b0), cx<T>(a1, (T)0), b1); ge = (T)k.gzr; }
-    else { Je = cur_L<T>(-b0, cx<T>(a0, (T)0), -conj_(b1), cx<T>(a1, (T)0)); ge = (T)k.gzl; }
-    if (h3) { Jm = cur_R<T>(cx<T>(a3, (T)0), conj_(b3), cx<T>(-a2, (T)0), -b2); gm = (T)k.gzr; }
-    else { Jm = cur_L<T>(-b3, cx<T>(a3, (T)0), -conj_(b2), cx<T>(a2, (T)0)); gm = (T)k.gzl; }
+    Vec4<T> Je, Jm;              // selected value by value: a reference into the event would force it into local memory
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+      Je.v[i] = cx<T>(h1 ? ev.JeR.v[i].re : ev.JeL.v[i].re, h1 ? ev.JeR.v[i].im : ev.JeL.v[i].im);
+      Jm.v[i] = cx<T>(h3 ? ev.JmR.v[i].re : ev.JmL.v[i].re, h3 ? ev.JmR.v[i].im : ev.JmL.v[i].im);
+    }
+    const cx<T> jeq(h1 ? ev.qeR.re : ev.qeL.re, h1 ? ev.qeR.im : ev.qeL.im), jmq(h3 ? ev.qmR.re : ev.qmL.re, h3 ? ev.qmR.im : ev.qmL.im);
+    const T ge = h1 ? (T)k.gzr : (T)k.gzl, gm = h3 ? (T)k.gzr : (T)k.gzl;
     const T e = (T)k.ee;
-    const cx<T> jj = mdot(Je, Jm), jeq = mdot(Je, ev.q), jmq = mdot(Jm, ev.q);
+    const cx<T> jj = mdot(Je, Jm);
     const cx<T> zc = (ge * gm) * ev.bw;                                    // Z exchange: couplings x Breit-Wigner
     const cx<T> coef = cx<T>(fma_<T>(e * e, ev.is, zc.re), zc.im);          // photon + Z on the g^{mu nu} part
     const cx<T> amp = coef * jj - (zc * ((T)1 / (T)k.mZ2)) * (jeq * jmq);

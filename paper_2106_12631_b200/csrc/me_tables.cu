@@ -6,13 +6,13 @@
 
 namespace mg {
 
-// e+ e- -> mu+ mu-: hand tally of eemumu.cuh.  Per NON-VANISHING helicity combination: two
-// single-chirality currents (4 complex products + 4 complex sums = 32 each), J_e.J_m (30), J_e.q and J_m.q (14 each), the
-// photon + Z coefficient (2 + 3 + 1), the two terms of the amplitude (6 + 2 + 6 + 6 + 2), the square (3); the
-// external spinors are selections of the per-event frames (no arithmetic).
-// Per event: s, 1/s, Breit-Wigner (20) and 4 massless spinor frames (pT^2 3, P 4, P+pz 2, rsqrt 2, 3 products = 14 each).
-static const int kFlopsPerHelicity_ee = 2 * 32 + 30 + 2 * 14 + 6 + 22 + 3;
-static const int kFlopsFixed_ee = 4 + 7 + 1 + 1 + 4 + 3 + 4 * 14;
+// e+ e- -> mu+ mu-: hand tally of eemumu.cuh.  Per NON-VANISHING helicity combination:
+// J_e.J_m (30), the photon + Z coefficient (2 + 3 + 1), the two terms of the amplitude (6 + 2 + 6 + 6 + 2), the square (3).
+// Per event: s, 1/s, Breit-Wigner (20), 4 massless spinor frames (pT^2 3, P 4, P+pz 2, rsqrt 2, 3 products = 14 each), the
+// four single-chirality currents every helicity combination selects from (4 complex products + 4 complex sums = 32 each)
+// and their contractions with q (14 each).
+static const int kFlopsPerHelicity_ee = 30 + 6 + 22 + 3;      // J_e . J_m, couplings, amplitude, |.|^2: the currents are per event
+static const int kFlopsFixed_ee = 4 + 7 + 1 + 1 + 4 + 3 + 4 * 14 + 4 * 32 + 4 * 14;      // + the four currents and their contractions with q
 
 int64_t me_flops_per_helicity(int process) {
   switch (process) {
