@@ -21,9 +21,13 @@ struct Eemumu {
   static constexpr int NHEL = 16;
   static constexpr int NPAR = 4;
   static constexpr bool FLIP = false;   // chiral Z couplings: |M(h)|^2 != |M(-h)|^2
-  // resident CTAs of 128 threads the register allocation aims at (measured on B200, 2^24 events): FP32 6 (64 registers, no
-  // spills: 0.408 ms); FP64 holds the four currents in 64 registers: 5 CTAs (96 registers) 0.735 ms, 4 (122) 0.756, 6 (80) 0.872
-  static constexpr int MINB = 6, MINB64 = 5;
+  static constexpr int MINB = 6;            // resident CTAs of 128 threads the register allocation aims at
+  // Where the two single-chirality currents of a helicity combination are evaluated.  Each line has ONE non-zero helicity
+  // assignment per chirality, so the 16 combinations share four currents and their four contractions with q.  FP32 evaluates
+  // them once per event (696 -> 504 flops per event: 0.47 -> 0.41 ms per 2^24 events).  FP64 keeps them inside the
+  // helicity loop: four currents are 64 registers in double, which costs a resident CTA or spills — measured in bench.py's
+  // step 0.77 (5 CTAs, 96 registers) / 0.82 ms (4 CTAs, 122) against 0.76 ms with the currents in the loop (6 CTAs, 80).
+  template <class T> static constexpr bool per_event_currents() { return sizeof(T) == 4; }
   // Massless helicity spinors need three reals per particle (the "simplified" IXXXXX/OXXXXX of PAPER.md:136):
   //   omega_+ chi_+ = (a, b),  omega_+ chi_- = (-b^*, a),   a = sqrt(P+pz),  b = (px + i py)/sqrt(P+pz),
   // P+pz evaluated as pT^2/(P-pz) for pz < 0 (R19); along -z: a = 0, b = sqrt(2P) (B1).  One square root, one
@@ -31,7 +35,7 @@ struct Eemumu {
   // Each of the two currents has ONE non-zero helicity assignment per chirality, so all 16 helicity combinations share
   // four currents and their four contractions with q: they are evaluated once per event (finish), and a helicity
   // combination only selects one of each and does the final contraction (helicity)
-  template <class T> struct Event { Mom<T> p[4]; Mom<T> q; T is; cx<T> bw; Vec4<T> JeR, JeL, JmR, JmL; cx<T> qeR, qeL, qmR, qmL; };
+  template <class T> struct Event { Mom<T> p[4]; Mom<T> q; T is; cx<T> bw; T a[4]; cx<T> b[4]; Vec4<T> JeR, JeL, JmR, JmL; cx<T> qeR, qeL, qmR, qmL; };
 
   template <class T> static MG_HD void massless_frame(Mom<T> p, T& a, cx<T>& b) {
     const T px = p.v[1], py = p.v[2], pz = p.v[3];
@@ -56,10 +60,11 @@ struct Eemumu {
     const T dr = s - (T)k.mZ2, di = (T)k.mZgZ;
     const T inv = (T)1 / fma_<T>(dr, dr, di * di);
     ev.bw = cx<T>(dr * inv, -di * inv);
-    T a0, a1, a2, a3;
-    cx<T> b0, b1, b2, b3;
-    massless_frame<T>(ev.p[0], a0, b0); massless_frame<T>(ev.p[1], a1, b1);
-    massless_frame<T>(ev.p[2], a2, b2); massless_frame<T>(ev.p[3], a3, b3);
+#pragma unroll
+    for (int i = 0; i < 4; ++i) massless_frame<T>(ev.p[i], ev.a[i], ev.b[i]);
+    if (!per_event_currents<T>()) return;
+    const T a0 = ev.a[0], a1 = ev.a[1], a2 = ev.a[2], a3 = ev.a[3];
+    const cx<T> b0 = ev.b[0], b1 = ev.b[1], b2 = ev.b[2], b3 = ev.b[3];
     // the e+ e- current and the mu+ mu- current vanish unless the two helicities of a line are opposite, and each is a
     // single chirality block:
     //   vbar(e+, h0) gamma^mu u(e-, h1):   h1 = +1: a = (-a0, -b0^*), psi_R = (a1, b1)       h1 = -1: b = (-b0, a0), psi_L = (-b1^*, a1)
@@ -94,13 +99,26 @@ struct Eemumu {
   template <class T> static MG_HD T helicity(const Event<T>& ev, int ihel, const Consts& k) {
     const bool h0 = (ihel & 1) != 0, h1 = (ihel & 2) != 0, h2 = (ihel & 4) != 0, h3 = (ihel & 8) != 0;
     if (h0 == h1 || h2 == h3) return (T)0;
-    Vec4<T> Je, Jm;              // selected value by value: a reference into the event would force it into local memory
+    Vec4<T> Je, Jm;
+    cx<T> jeq, jmq;
+    if (per_event_currents<T>()) {
+      // selected value by value: a reference into the event would force it into local memory
 #pragma unroll
-    for (int i = 0; i < 4; ++i) {
-      Je.v[i] = cx<T>(h1 ? ev.JeR.v[i].re : ev.JeL.v[i].re, h1 ? ev.JeR.v[i].im : ev.JeL.v[i].im);
-      Jm.v[i] = cx<T>(h3 ? ev.JmR.v[i].re : ev.JmL.v[i].re, h3 ? ev.JmR.v[i].im : ev.JmL.v[i].im);
+      for (int i = 0; i < 4; ++i) {
+        Je.v[i] = cx<T>(h1 ? ev.JeR.v[i].re : ev.JeL.v[i].re, h1 ? ev.JeR.v[i].im : ev.JeL.v[i].im);
+        Jm.v[i] = cx<T>(h3 ? ev.JmR.v[i].re : ev.JmL.v[i].re, h3 ? ev.JmR.v[i].im : ev.JmL.v[i].im);
+      }
+      jeq = cx<T>(h1 ? ev.qeR.re : ev.qeL.re, h1 ? ev.qeR.im : ev.qeL.im);
+      jmq = cx<T>(h3 ? ev.qmR.re : ev.qmL.re, h3 ? ev.qmR.im : ev.qmL.im);
+    } else {
+      const T a0 = ev.a[0], a1 = ev.a[1], a2 = ev.a[2], a3 = ev.a[3];
+      const cx<T> b0 = ev.b[0], b1 = ev.b[1], b2 = ev.b[2], b3 = ev.b[3];
+      if (h1) Je = cur_R<T>(cx<T>(-a0, (T)0), -conj_(b0), cx<T>(a1, (T)0), b1);
+      else Je = cur_L<T>(-b0, cx<T>(a0, (T)0), -conj_(b1), cx<T>(a1, (T)0));
+      if (h3) Jm = cur_R<T>(cx<T>(a3, (T)0), conj_(b3), cx<T>(-a2, (T)0), -b2);
+      else Jm = cur_L<T>(-b3, cx<T>(a3, (T)0), -conj_(b2), cx<T>(a2, (T)0));
+      jeq = mdot(Je, ev.q); jmq = mdot(Jm, ev.q);
     }
-    const cx<T> jeq(h1 ? ev.qeR.re : ev.qeL.re, h1 ? ev.qeR.im : ev.qeL.im), jmq(h3 ? ev.qmR.re : ev.qmL.re, h3 ? ev.qmR.im : ev.qmL.im);
     const T ge = h1 ? (T)k.gzr : (T)k.gzl, gm = h3 ? (T)k.gzr : (T)k.gzl;
     const T e = (T)k.ee;
     const cx<T> jj = mdot(Je, Jm);

@@ -12,7 +12,7 @@
 namespace mg {
 
 template <class Proc, class T, int NF, bool MASSIVE>
-__global__ void __launch_bounds__(kMeThreads, MinBlocks<Proc, T>::value) fused_kernel(Consts k, uint64_t seed, uint64_t first, int64_t n,
+__global__ void __launch_bounds__(kMeThreads, Proc::MINB) fused_kernel(Consts k, uint64_t seed, uint64_t first, int64_t n,
                                                            T* __restrict__ me, T* __restrict__ psw, T* __restrict__ evw,
                                                            uint64_t mask) {
   static_assert(Proc::NPAR == NF + 2, "two beams + NF final particles");

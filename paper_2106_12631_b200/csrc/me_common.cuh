@@ -21,11 +21,6 @@ constexpr int kMeThreads = 128;
 // colour-summed |M|^2 of helicity combination h equals that of its complement NHEL-1-h at the SAME momenta.  Proc::FLIP
 // processes evaluate one member of each pair (the one with the last particle at helicity -1) and count it once per
 // member that the good-helicity mask keeps.  Not for e+ e- -> mu+ mu- (the Z couplings are chiral).
-// resident CTAs per SM the register allocation aims at: Proc::MINB, or Proc::MINB64 for the double-precision kernels of a
-// process that declares it (twice the registers per value: a lower target avoids spills)
-template <class Proc, class T, class = void> struct MinBlocks { static constexpr int value = Proc::MINB; };
-template <class Proc> struct MinBlocks<Proc, double, decltype((void)Proc::MINB64)> { static constexpr int value = Proc::MINB64; };
-
 template <class Proc> MG_HD uint64_t flip_half(uint64_t mask) {
   if (!Proc::FLIP) return mask;
   uint64_t rev = 0;
@@ -43,7 +38,7 @@ template <class Proc> MG_HD int flip_weight(uint64_t mask, int h) {
 //   static int    NHEL, NPAR
 // mask: good helicities (bit h).  me = norm * sum_h.  PER_HEL: write every helicity, ignore mask.
 template <class Proc, class T, bool PER_HEL>
-__global__ void __launch_bounds__(kMeThreads, MinBlocks<Proc, T>::value) sigmakin_kernel(Consts k, const T* __restrict__ mom, int64_t n, int64_t ld,
+__global__ void __launch_bounds__(kMeThreads, Proc::MINB) sigmakin_kernel(Consts k, const T* __restrict__ mom, int64_t n, int64_t ld,
                                                               T* __restrict__ me, const T* __restrict__ psw,
                                                               T* __restrict__ evw, T* __restrict__ hel_out, uint64_t mask) {
   const int64_t e = (int64_t)blockIdx.x * kMeThreads + threadIdx.x;

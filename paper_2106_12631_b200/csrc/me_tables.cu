@@ -6,17 +6,19 @@
 
 namespace mg {
 
-// e+ e- -> mu+ mu-: hand tally of eemumu.cuh.  Per NON-VANISHING helicity combination:
-// J_e.J_m (30), the photon + Z coefficient (2 + 3 + 1), the two terms of the amplitude (6 + 2 + 6 + 6 + 2), the square (3).
-// Per event: s, 1/s, Breit-Wigner (20), 4 massless spinor frames (pT^2 3, P 4, P+pz 2, rsqrt 2, 3 products = 14 each), the
-// four single-chirality currents every helicity combination selects from (4 complex products + 4 complex sums = 32 each)
-// and their contractions with q (14 each).
-static const int kFlopsPerHelicity_ee = 30 + 6 + 22 + 3;      // J_e . J_m, couplings, amplitude, |.|^2: the currents are per event
-static const int kFlopsFixed_ee = 4 + 7 + 1 + 1 + 4 + 3 + 4 * 14 + 4 * 32 + 4 * 14;      // + the four currents and their contractions with q
+// e+ e- -> mu+ mu-: hand tally of eemumu.cuh.  The two single-chirality currents of a
+// helicity combination (4 complex products + 4 complex sums = 32 each) and their contractions with q (14 each) are inside
+// the helicity loop in FP64 and per event (four currents, four contractions) in FP32 (eemumu.cuh per_event_currents).
+// Per NON-VANISHING helicity combination besides: J_e.J_m (30), the photon + Z coefficient (2 + 3 + 1), the two terms of the
+// amplitude (6 + 2 + 6 + 6 + 2), the square (3).  Per event: s, 1/s, Breit-Wigner (20) and 4 massless spinor frames
+// (pT^2 3, P 4, P+pz 2, rsqrt 2, 3 products = 14 each).
+static const int kFlopsPerHelicity_ee = 30 + 6 + 22 + 3;
+static const int kFlopsCurrents_ee = 2 * 32 + 2 * 14;      // one pair of currents with their q contractions
+static const int kFlopsFixed_ee = 4 + 7 + 1 + 1 + 4 + 3 + 4 * 14;
 
-int64_t me_flops_per_helicity(int process) {
+int64_t me_flops_per_helicity(int process, bool fp64) {
   switch (process) {
-    case MG_EEMUMU: return kFlopsPerHelicity_ee;
+    case MG_EEMUMU: return kFlopsPerHelicity_ee + (fp64 ? kFlopsCurrents_ee : 0);
     case MG_GGTT: return kFlopsPerHelicity_2;
     case MG_GGTTG: return kFlopsPerHelicity_3;
     case MG_GGTTGG: return kFlopsPerHelicity_4;
@@ -25,9 +27,9 @@ int64_t me_flops_per_helicity(int process) {
   }
   return 0;
 }
-int64_t me_flops_per_event_fixed(int process) {
+int64_t me_flops_per_event_fixed(int process, bool fp64) {
   switch (process) {
-    case MG_EEMUMU: return kFlopsFixed_ee;
+    case MG_EEMUMU: return kFlopsFixed_ee + (fp64 ? 0 : 2 * kFlopsCurrents_ee);
     case MG_GGTT: return kFlopsFixed_2;
     case MG_GGTTG: return kFlopsFixed_3;
     case MG_GGTTGG: return kFlopsFixed_4;

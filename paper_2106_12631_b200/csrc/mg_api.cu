@@ -579,7 +579,8 @@ int64_t mg_flops_per_event(const mg_process* p, int stage) {
       for (int h = 0; h < p->n_hel / 2; ++h) half |= (((p->hel_mask >> h) | (p->hel_mask >> (p->n_hel - 1 - h))) & 1ull) << h;
       good = __builtin_popcountll(half);
     }
-    return me_flops_per_event_fixed(p->par.process) + (int64_t)good * me_flops_per_helicity(p->par.process);
+    const bool f64 = p->par.precision == MG_FP64;
+    return me_flops_per_event_fixed(p->par.process, f64) + (int64_t)good * me_flops_per_helicity(p->par.process, f64);
   }
   return 0;  // the RNG and RAMBO stages are HBM-bound; their roofline is bytes (mg_bytes_per_event)
 }

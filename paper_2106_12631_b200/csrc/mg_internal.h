@@ -103,8 +103,8 @@ int64_t unweight_tiles(int64_t n);
 cudaError_t launch_unweight(const mg_process* p, uint64_t seed, uint64_t first, const void* d_w, int64_t n, double wmax,
                             unsigned long long* d_state, int64_t* d_out, int64_t* d_count, cudaStream_t s);
 // explicit flop tally of one helicity combination / fixed per-event overhead (generated)
-int64_t me_flops_per_helicity(int process);
-int64_t me_flops_per_event_fixed(int process);
+int64_t me_flops_per_helicity(int process, bool fp64);
+int64_t me_flops_per_event_fixed(int process, bool fp64);
 int64_t me_flops_per_event_recycle(int process, bool fp64);   // >= 0: the process runs the recycling kernel
 // colour matrix numerators / denominator (generated tables), row-major n_flows x n_flows
 const int* me_colour_numerators(int process, int* denom_out);
