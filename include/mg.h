@@ -114,8 +114,9 @@ int mg_generate(mg_process* p, uint64_t seed, uint64_t first_event, int64_t n, i
  * element of events first_event .. first_event+n-1 without the momenta ever being stored: ONE launch for every
  * process.  Writes me[n] and, if non-NULL, ps_weight[n] and event_weight[n] = ps_weight * me (R18); uses the
  * installed helicity mask.  e+e- -> mu+mu- and g g -> t t~ keep everything in registers; in the shared-memory kernels
- * of g g -> t t~ g(g) one thread per event of the CTA generates the momenta into shared memory before the first step.
- * Asynchronous on `stream`.  Same values as mg_generate + mg_sigmakin up to rounding of contracted multiply-adds.
+ * of g g -> t t~ g(g) four lanes per event of the CTA generate the momenta into shared memory before the first step.
+ * Asynchronous on `stream`.  Same values as mg_generate + mg_sigmakin up to rounding of contracted multiply-adds (the
+ * shared-memory kernels: the same bits).
  * Errors: MG_EINVAL (NULL/misaligned d_me, bad handle, n < 0), MG_ENOMEM, MG_ECUDA. */
 int mg_sigmakin_fused(mg_process* p, uint64_t seed, uint64_t first_event, int64_t n,
                       void* d_me, void* d_ps_weight, void* d_event_weight, void* stream);

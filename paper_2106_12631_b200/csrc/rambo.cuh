@@ -154,4 +154,100 @@ MG_HD T rambo_finish(const T (&q0)[NF], const T (&nx)[NF], const T (&ny)[NF], co
   return w;
 }
 
+
+#ifdef __CUDACC__
+// rambo_finish spread over the final particles of an event: FOUR consecutive lanes of a warp hold one event, lane i < NF
+// owns particle i (its direction and energy from rambo_direction; lanes i >= NF carry a copy of particle 0 and only take
+// part in the exchanges).  Everything that depends on one particle — its reciprocal square root in every Newton step, its
+// boosted momentum, its final square root and divisions — is evaluated by its lane only; the sums over particles are
+// gathered with shuffles and added IN THE ORDER OF rambo_finish, so the momenta and the weight are the same bits as
+// mg_generate's.  Used by the shared-memory kernels in M_GEN mode (recycle.cuh), where the CTA waits for this chain:
+// a third of the instructions of the one-thread form on the critical path.  All 32 lanes of the warp must call it.
+// p: the lane's particle (E, px, py, pz); returns the phase-space weight (the same in the four lanes of an event).
+template <class T, int NF>
+__device__ __forceinline__ T rambo_finish_lanes(int i, T q0m, T nxm, T nym, T nzm, const Consts& k, T (&p)[4]) {
+  static_assert(NF <= 4, "four lanes per event");
+  const unsigned full = 0xffffffffu;
+  T q0[NF], nx[NF], ny[NF], nz[NF];
+#pragma unroll
+  for (int j = 0; j < NF; ++j) {
+    q0[j] = __shfl_sync(full, q0m, j, 4); nx[j] = __shfl_sync(full, nxm, j, 4);
+    ny[j] = __shfl_sync(full, nym, j, 4); nz[j] = __shfl_sync(full, nzm, j, 4);
+  }
+  T Q0 = 0;
+#pragma unroll
+  for (int j = 0; j < NF; ++j) Q0 += q0[j];
+  // h_ij of the lane's particle with every other one ((-a)^2 = a^2: the value rambo_finish uses for either order of i, j)
+  T hm[NF];
+#pragma unroll
+  for (int j = 0; j < NF; ++j) {
+    const T dx = nxm - nx[j], dy = nym - ny[j], dz = nzm - nz[j];
+    hm[j] = (T)0.5 * fma_<T>(dx, dx, fma_<T>(dy, dy, dz * dz));
+  }
+  T gm = 0;
+#pragma unroll
+  for (int j = 0; j < NF; ++j) gm = (j != i) ? fma_<T>(q0[j], hm[j], gm) : gm;
+  T g[NF];
+  T M2 = 0;
+#pragma unroll
+  for (int j = 0; j < NF; ++j) { g[j] = __shfl_sync(full, gm, j, 4); M2 = fma_<T>(q0[j], g[j], M2); }
+  const T sqrt_s = (T)k.sqrt_s;
+  const T M = sqrt_<T>(M2);
+  const T x = sqrt_s / M;
+  const T xD = x / (M * (M + Q0));
+  const T e0 = sqrt_s / M2;
+  T sx = 0, sy = 0, sz = 0;
+#pragma unroll
+  for (int j = 0; j < NF; ++j) {
+    const T a = q0[j] * (M + g[j]), b = q0[j] * (g[j] - gm);
+    const T tx = fma_<T>(a, nxm - nx[j], fma_<T>(b, nx[j], sx));
+    const T ty = fma_<T>(a, nym - ny[j], fma_<T>(b, ny[j], sy));
+    const T tz = fma_<T>(a, nzm - nz[j], fma_<T>(b, nz[j], sz));
+    if (j != i) { sx = tx; sy = ty; sz = tz; }
+  }
+  const T f0 = xD * q0m;
+  p[0] = e0 * q0m * gm;
+  p[1] = f0 * sx; p[2] = f0 * sy; p[3] = f0 * sz;
+  // massive rescaling: Newton as in rambo_finish; the lane contributes sqrt(m^2 + xi^2 p0^2) of its particle
+  T summ = 0;
+#pragma unroll
+  for (int j = 0; j < NF; ++j) summ += (T)k.mass[j];
+  T mm = 0;
+#pragma unroll
+  for (int j = 0; j < NF; ++j) mm = (j == i) ? (T)k.mass[j] : mm;
+  const T m2m = mm * mm, p02m = p[0] * p[0];
+  const T r = summ / sqrt_s;
+  T xi = sqrt_<T>((T)1 - r * r);
+  const T tol = (sizeof(T) == 8 ? (T)3.6e-15 : (T)1.9e-6) * sqrt_s;
+#pragma unroll 1
+  for (int it = 0; it < 8; ++it) {
+    const T argm = fma_<T>(xi * xi, p02m, m2m);
+    const T invm = rsqrt_<T>(argm);
+    const T dm = xi * p02m;
+    T f = -sqrt_s, df = 0;
+#pragma unroll
+    for (int j = 0; j < NF; ++j) {
+      const T arg = __shfl_sync(full, argm, j, 4), inv = __shfl_sync(full, invm, j, 4), d = __shfl_sync(full, dm, j, 4);
+      f = fma_<T>(arg, inv, f);
+      df = fma_<T>(d, inv, df);
+    }
+    const bool done = abs_<T>(f) <= tol;
+    if (!done) xi -= f / df;
+    if (__all_sync(full, done)) break;
+  }
+  const T kabsm = xi * p[0];
+  const T Em = sqrt_<T>(fma_<T>(kabsm, kabsm, m2m));
+  p[0] = Em;
+  p[1] *= xi; p[2] *= xi; p[3] *= xi;
+  const T ratm = kabsm / Em, s2m = kabsm * kabsm / Em;
+  T prod = 1, sum2 = 0;
+#pragma unroll
+  for (int j = 0; j < NF; ++j) { prod *= __shfl_sync(full, ratm, j, 4); sum2 += __shfl_sync(full, s2m, j, 4); }
+  T xipow = 1;
+#pragma unroll
+  for (int j = 0; j < 2 * NF - 3; ++j) xipow *= xi;
+  return (T)k.w0 * xipow * prod * sqrt_s / sum2;
+}
+#endif
+
 }  // namespace mg

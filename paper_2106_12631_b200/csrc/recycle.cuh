@@ -83,7 +83,7 @@ template <int MASK> __device__ __forceinline__ int pextc(int v) {
 //   M_PERHEL  write |M|^2 of every helicity combination instead of the sum (good-helicity filter, parity tests)
 //   M_GATHER  the CTA's events are taken from a list of event indices written by an earlier launch (the double-
 //             precision pass over the ill-conditioned events of an FP32 batch); persistent grid
-//   M_GEN     the momenta are not read but GENERATED by the CTA (Philox -> RAMBO, one thread per event) into shared
+//   M_GEN     the momenta are not read but GENERATED by the CTA (Philox -> RAMBO, four lanes per event) into shared
 //             memory: mg_sigmakin_fused, A1-A13 in one launch, momenta never in HBM
 //   M_SPLIT   kernel A of the two-kernel form (split.cuh, "many smaller kernels ... CUDA graphs"): stop after
 //             the colour-flow sums J_f and write them to a.jamp; colour and helicity sums are kernel B's
@@ -396,34 +396,30 @@ __device__ __forceinline__ void rc_batch(unsigned char* smem_raw, const Consts& 
     }
     __syncthreads();
     if (GEN) {
-      // A1-A3 spread over the CTA: thread (event, final particle) draws the particle's four uniforms and evaluates its
-      // direction and energy (the transcendental part of RAMBO, rambo.cuh); one thread per event then does the rest
-      // in the order of rambo_core, so the momenta are those of mg_generate bit for bit
+      // A1-A4 on four lanes per event: lane i < NF draws the four Philox uniforms of final particle i and evaluates its
+      // direction and energy (the transcendental part of RAMBO, rambo.cuh), then the lanes of an event finish RAMBO
+      // together (rambo_finish_lanes: every sum in the order of rambo_core, so the momenta are those of mg_generate bit
+      // for bit); the CTA waits for this chain, which is why it is spread over the particles
       constexpr int NF = P::NPAR - 2;
-      TI* dirs = reinterpret_cast<TI*>(s.ent);              // [E][NF][4] (q0, nx, ny, nz): the entry table is not in use yet
-      if (tid < P::E * NF) {
-        const int e = tid / NF, i = tid - e * NF;
-        const u32x4 r = philox_event_particle(a.seed, a.first + (uint64_t)evidx[e], (uint32_t)i);
+      static_assert((P::E * 4) % 32 == 0 && P::E * 4 <= P::NT, "whole warps generate the momenta");
+      if (tid < P::E * 4) {
+        const int e = tid >> 2, i = tid & 3;
+        const u32x4 r = philox_event_particle(a.seed, a.first + (uint64_t)evidx[e], (uint32_t)(i < NF ? i : 0));
         TI q0, nx, ny, nz;
         rambo_direction<TI>(u32_to_uniform<TI>(r.x), u32_to_uniform<TI>(r.y), u32_to_uniform<TI>(r.z), u32_to_uniform<TI>(r.w), q0, nx, ny, nz);
-        TI* o = dirs + (e * NF + i) * 4;
-        o[0] = q0; o[1] = nx; o[2] = ny; o[3] = nz;
-      }
-      __syncthreads();
-      if (tid < P::E) {
-        TI q0[NF], nx[NF], ny[NF], nz[NF];
+        TI pf[4];
+        const TI w = rambo_finish_lanes<TI, NF>(i, q0, nx, ny, nz, k, pf);
+        T* o = s.pext + e * P::NPAR * 4;
+        if (i < NF) {
 #pragma unroll
-        for (int i = 0; i < NF; ++i) { const TI* o = dirs + (tid * NF + i) * 4; q0[i] = o[0]; nx[i] = o[1]; ny[i] = o[2]; nz[i] = o[3]; }
-        TI pf[NF][4];
-        wps[tid] = rambo_finish<TI, NF, true>(q0, nx, ny, nz, k, pf);
-        T* o = s.pext + tid * P::NPAR * 4;
-        const T hs = (T)((TI)0.5 * (TI)k.sqrt_s);          // beams (R5), as rambo_event writes them
-        o[0] = hs; o[1] = (T)0; o[2] = (T)0; o[3] = hs;
-        o[4] = hs; o[5] = (T)0; o[6] = (T)0; o[7] = -hs;
-#pragma unroll
-        for (int i = 0; i < NF; ++i)
-#pragma unroll
-          for (int mu = 0; mu < 4; ++mu) o[8 + 4 * i + mu] = (T)pf[i][mu];
+          for (int mu = 0; mu < 4; ++mu) o[8 + 4 * i + mu] = (T)pf[mu];
+        }
+        if (i == 0) {
+          wps[e] = w;
+          const T hs = (T)((TI)0.5 * (TI)k.sqrt_s);          // beams (R5), as rambo_event writes them
+          o[0] = hs; o[1] = (T)0; o[2] = (T)0; o[3] = hs;
+          o[4] = hs; o[5] = (T)0; o[6] = (T)0; o[7] = -hs;
+        }
       }
     } else {
       for (int t = tid; t < P::E * P::NPAR * 4; t += P::NT) {
