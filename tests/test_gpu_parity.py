@@ -614,6 +614,22 @@ def test_split_kernels_under_a_graph_give_the_same_values(mg, process, prec, n, 
         mg.Process(1, 0).sigmakin_split(mom, n, me=me)
 
 
+@pytest.mark.parametrize("process,prec", [(2, 0), (2, 1), (3, 0), (3, 1)])
+def test_fused_shared_memory_kernels_give_the_bits_of_the_separate_launches(mg, process, prec):
+    """mg_sigmakin_fused of g g -> t t~ g (g): four lanes per event finish RAMBO together (rambo.cuh rambo_finish_lanes), every
+    sum over particles in the order of the one-thread form, so phase-space weights, matrix elements and event weights are the
+    same bits as mg_generate + mg_sigmakin — on whole CTAs, a ragged tail and a range that starts at a large event index."""
+    P = mg.Process(process, prec)
+    for first, n in ((0, 4096 + 13), (3 << 40, 777)):
+        mom, w = P.generate(7, first, n)
+        ew_s = torch.empty(mom.shape[1], dtype=P.dtype, device="cuda")
+        me_s = P.sigmakin(mom, n, ps_weight=w, event_weight=ew_s)
+        w_f = torch.empty(n, dtype=P.dtype, device="cuda")
+        ew_f = torch.empty(n, dtype=P.dtype, device="cuda")
+        me_f = P.sigmakin_fused(7, first, n, None, w_f, ew_f)
+        assert torch.equal(w_f, w[:n]) and torch.equal(me_f[:n], me_s[:n]) and torch.equal(ew_f, ew_s[:n])
+
+
 def test_sharded_sums_on_one_device(mg):
     """shard.gpu_compute (the compute leg of the multi-GPU path) on one device: world 1 and two
     emulated ranks (rank/world passed explicitly) merge to the same sums, which match the oracle on the same events."""
