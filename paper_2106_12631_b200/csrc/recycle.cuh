@@ -268,7 +268,14 @@ template <class P, class T_, class TI_, int MODE> struct Smem {
   static constexpr int kEvStride = 4 * P::NSLOT + 64 / (int)sizeof(W);
   static constexpr size_t kRedOff = kEntOff + (size_t)P::E * kEvStride * sizeof(W);
   static constexpr size_t kIdxOff = (kRedOff + (P::NT / 32) * sizeof(T) + 15) / 16 * 16;
-  static constexpr size_t bytes() { return kIdxOff + (STAGED ? (size_t)P::E * 16 : 0) + 16; }
+  // M_GEN: a CTA generates the momenta of NB batches of E events up front (one or two warps per batch, side by side) and
+  // then runs the batches one after the other: the wait for the RAMBO chain is paid once per NB batches (P::GENB / GENB32,
+  // gen/recycle.py: 2 for g g -> t t~ g in FP64, else 1).  Batch 0 uses the regions above; batch b > 0 has its own [pext T[E][NPAR][4]] [event indices int64[E]] [weights TI[E]] after them.
+  static constexpr int NB = (MODE == M_GEN) ? (sizeof(T) == 8 ? P::GENB : P::GENB32) : 1;
+  static constexpr size_t kSlotOff = kIdxOff + (STAGED ? (size_t)P::E * 16 : 0) + 16;
+  static constexpr size_t kSlotPext = ((size_t)P::E * P::NPAR * 4 * sizeof(T) + 15) / 16 * 16;
+  static constexpr size_t kSlotBytes = kSlotPext + (size_t)P::E * 16;
+  static constexpr size_t bytes() { return kSlotOff + (size_t)(NB - 1) * kSlotBytes; }
   __device__ __forceinline__ void bind(unsigned char* raw) {
     pext4 = reinterpret_cast<unsigned long long*>(raw);
     mom = reinterpret_cast<T*>(raw + 128);
@@ -277,8 +284,14 @@ template <class P, class T_, class TI_, int MODE> struct Smem {
     ent = reinterpret_cast<W*>(raw + kEntOff);
     red = reinterpret_cast<T*>(raw + kRedOff);
   }
-  static __device__ __forceinline__ int64_t* evidx(unsigned char* raw) { return reinterpret_cast<int64_t*>(raw + kIdxOff); }
-  static __device__ __forceinline__ TI* wps(unsigned char* raw) { return reinterpret_cast<TI*>(raw + kIdxOff + (size_t)P::E * 8); }
+  static __device__ __forceinline__ unsigned char* slot_base(unsigned char* raw, int slot) { return raw + kSlotOff + (size_t)(slot - 1) * kSlotBytes; }
+  static __device__ __forceinline__ int64_t* evidx(unsigned char* raw, int slot = 0) {
+    return reinterpret_cast<int64_t*>(slot ? slot_base(raw, slot) + kSlotPext : raw + kIdxOff);
+  }
+  static __device__ __forceinline__ TI* wps(unsigned char* raw, int slot = 0) {
+    return reinterpret_cast<TI*>((slot ? slot_base(raw, slot) + kSlotPext : raw + kIdxOff) + (size_t)P::E * 8);
+  }
+  __device__ __forceinline__ void use_slot(unsigned char* raw, int slot) { if (slot) pext = reinterpret_cast<T*>(slot_base(raw, slot)); }
   __device__ __forceinline__ VW view(int e) const {
     VW v;
     v.gm = gmom + (e < nev ? e : nev - 1); v.gld = ld;     // tail events re-read the last event and are not stored
@@ -369,9 +382,37 @@ template <class P, class SM> __device__ __forceinline__ void run_momtab(const SM
 // ---------------------------------------------------------------------------------------------------
 // the kernel: grid = ceil(n / E) CTAs of NT = E * NHEL threads (M_GATHER: a persistent grid over the list)
 // ---------------------------------------------------------------------------------------------------
+// A1-A4 on four lanes per event (M_GEN): lane i < NF of event e draws the four Philox uniforms of final particle i and
+// evaluates its direction and energy (the transcendental part of RAMBO, rambo.cuh), then the lanes of an event finish RAMBO
+// together (rambo_finish_lanes: every sum in the order of rambo_core, so the momenta are those of mg_generate bit for bit).
+// The CTA waits for this chain, which is why it is spread over the particles.  ltid = 4 e + i for e < E: whole warps.
+template <class P, class T, class TI>
+__device__ __forceinline__ void gen_momenta(int ltid, int64_t event, T* pext, TI* wps, const Consts& k, const RcArgs<TI>& a) {
+  constexpr int NF = P::NPAR - 2;
+  static_assert((P::E * 4) % 32 == 0 && P::E * 4 <= P::NT, "whole warps generate the momenta");
+  const int e = ltid >> 2, i = ltid & 3;
+  const u32x4 r = philox_event_particle(a.seed, a.first + (uint64_t)event, (uint32_t)(i < NF ? i : 0));
+  TI q0, nx, ny, nz;
+  rambo_direction<TI>(u32_to_uniform<TI>(r.x), u32_to_uniform<TI>(r.y), u32_to_uniform<TI>(r.z), u32_to_uniform<TI>(r.w), q0, nx, ny, nz);
+  TI pf[4];
+  const TI w = rambo_finish_lanes<TI, NF>(i, q0, nx, ny, nz, k, pf);
+  T* o = pext + e * P::NPAR * 4;
+  if (i < NF) {
+#pragma unroll
+    for (int mu = 0; mu < 4; ++mu) o[8 + 4 * i + mu] = (T)pf[mu];
+  }
+  if (i == 0) {
+    wps[e] = w;
+    const T hs = (T)((TI)0.5 * (TI)k.sqrt_s);          // beams (R5), as rambo_event writes them
+    o[0] = hs; o[1] = (T)0; o[2] = (T)0; o[3] = hs;
+    o[4] = hs; o[5] = (T)0; o[6] = (T)0; o[7] = -hs;
+  }
+}
+
 // one batch of E events: events ev0 .. ev0 + E - 1 of `total` (of the caller's arrays, or of the list with M_GATHER)
 template <class P, class T, class TI, int MODE>
-__device__ __forceinline__ void rc_batch(unsigned char* smem_raw, const Consts& k, const RcArgs<TI>& a, int64_t ev0, int64_t total) {
+__device__ __forceinline__ void rc_batch(unsigned char* smem_raw, const Consts& k, const RcArgs<TI>& a, int64_t ev0, int64_t total,
+                                         int slot = 0, bool pregen = false) {
   typedef Smem<P, T, TI, MODE> SM;
   constexpr bool PER_HEL = (MODE & M_PERHEL) != 0, GATHER = (MODE & M_GATHER) != 0, GEN = (MODE & M_GEN) != 0;
   // FP32 batches: events whose propagators are close to a pole are listed for the double-precision pass
@@ -388,39 +429,17 @@ __device__ __forceinline__ void rc_batch(unsigned char* smem_raw, const Consts& 
   s.nev = (int)((total - ev0) < (int64_t)P::E ? (total - ev0) : (int64_t)P::E);
   if (SM::STAGED) {
     // A5 (M_GATHER) or A1-A4 (M_GEN): the external momenta of the CTA's events go to shared memory first
-    int64_t* evidx = SM::evidx(smem_raw);
-    TI* wps = SM::wps(smem_raw);
+    int64_t* evidx = SM::evidx(smem_raw, slot);
+    TI* wps = SM::wps(smem_raw, slot);
+    s.use_slot(smem_raw, slot);
+    if (!pregen) {
     if (tid < P::E) {
       const int e = tid < s.nev ? tid : s.nev - 1;
       evidx[tid] = GATHER ? a.rlist[ev0 + e] : ev0 + e;
     }
     __syncthreads();
     if (GEN) {
-      // A1-A4 on four lanes per event: lane i < NF draws the four Philox uniforms of final particle i and evaluates its
-      // direction and energy (the transcendental part of RAMBO, rambo.cuh), then the lanes of an event finish RAMBO
-      // together (rambo_finish_lanes: every sum in the order of rambo_core, so the momenta are those of mg_generate bit
-      // for bit); the CTA waits for this chain, which is why it is spread over the particles
-      constexpr int NF = P::NPAR - 2;
-      static_assert((P::E * 4) % 32 == 0 && P::E * 4 <= P::NT, "whole warps generate the momenta");
-      if (tid < P::E * 4) {
-        const int e = tid >> 2, i = tid & 3;
-        const u32x4 r = philox_event_particle(a.seed, a.first + (uint64_t)evidx[e], (uint32_t)(i < NF ? i : 0));
-        TI q0, nx, ny, nz;
-        rambo_direction<TI>(u32_to_uniform<TI>(r.x), u32_to_uniform<TI>(r.y), u32_to_uniform<TI>(r.z), u32_to_uniform<TI>(r.w), q0, nx, ny, nz);
-        TI pf[4];
-        const TI w = rambo_finish_lanes<TI, NF>(i, q0, nx, ny, nz, k, pf);
-        T* o = s.pext + e * P::NPAR * 4;
-        if (i < NF) {
-#pragma unroll
-          for (int mu = 0; mu < 4; ++mu) o[8 + 4 * i + mu] = (T)pf[mu];
-        }
-        if (i == 0) {
-          wps[e] = w;
-          const T hs = (T)((TI)0.5 * (TI)k.sqrt_s);          // beams (R5), as rambo_event writes them
-          o[0] = hs; o[1] = (T)0; o[2] = (T)0; o[3] = hs;
-          o[4] = hs; o[5] = (T)0; o[6] = (T)0; o[7] = -hs;
-        }
-      }
+      if (tid < P::E * 4) gen_momenta<P, T, TI>(tid, evidx[tid >> 2], s.pext, wps, k, a);
     } else {
       for (int t = tid; t < P::E * P::NPAR * 4; t += P::NT) {
         const int e = t / (P::NPAR * 4), r = t - e * (P::NPAR * 4);
@@ -428,6 +447,7 @@ __device__ __forceinline__ void rc_batch(unsigned char* smem_raw, const Consts& 
       }
     }
     __syncthreads();
+    }
   } else {
     // A5: the momenta are read straight from the caller's array by the tasks of step 0 (line momenta, external
     // wavefunctions): no staging copy and no barrier in front of the first step
@@ -445,7 +465,7 @@ __device__ __forceinline__ void rc_batch(unsigned char* smem_raw, const Consts& 
   }
   T me_h = P::template run<T>(s, tid, el, h, (T)k.mt);     // generated: producer steps + inner products + colour sum
   // index of this thread's event in the caller's arrays
-  const int64_t ge = SM::STAGED ? SM::evidx(smem_raw)[el] : ev0 + el;
+  const int64_t ge = SM::STAGED ? SM::evidx(smem_raw, slot)[el] : ev0 + el;
   const bool live = el < s.nev;
 
   // helicity-flip symmetry (P::FLIP, R35): the thread's combination h has the last particle at helicity -1; its
@@ -486,7 +506,7 @@ __device__ __forceinline__ void rc_batch(unsigned char* smem_raw, const Consts& 
     const TI r = (TI)(me_h * (T)k.me_norm);
     a.me[ge] = r;
     if (GEN) {
-      const TI w = SM::wps(smem_raw)[el];
+      const TI w = SM::wps(smem_raw, slot)[el];
       if (a.psw_out != nullptr) a.psw_out[ge] = w;
       if (a.evw != nullptr) a.evw[ge] = w * r;
     } else if (a.evw != nullptr) {
@@ -509,6 +529,45 @@ __global__ void __launch_bounds__(P::NT, sizeof(T) == 8 ? P::MINB : P::MINB32) s
     for (int64_t ev0 = (int64_t)blockIdx.x * P::E; ev0 < total; ev0 += (int64_t)gridDim.x * P::E) {
       rc_batch<P, T, TI, MODE>(smem_raw, k, a, ev0, total);
       __syncthreads();      // the next batch of the persistent grid overwrites the shared memory
+    }
+  } else if (MODE == M_GEN && Smem<P, T, TI, MODE>::NB > 1) {
+    // the momenta of NB batches first, each on its own warp(s), then the batches one after the other (Smem::NB)
+    typedef Smem<P, T, TI, MODE> SM;
+    const int64_t b0 = (int64_t)blockIdx.x * SM::NB;
+    const int slot = (int)threadIdx.x / (P::E * 4), ltid = (int)threadIdx.x - slot * (P::E * 4);
+    const int64_t gev0 = (b0 + slot) * P::E;
+    if (slot < SM::NB && gev0 < a.n) {
+      SM s;
+      s.bind(smem_raw);
+      s.use_slot(smem_raw, slot);
+      const int64_t left = a.n - gev0;
+      const int e = ltid >> 2;
+      const int64_t event = gev0 + ((int64_t)e < left ? e : (int)left - 1);     // tail events repeat the last one and are not stored
+      if ((ltid & 3) == 0) SM::evidx(smem_raw, slot)[e] = event;
+      gen_momenta<P, T, TI>(ltid, event, s.pext, SM::wps(smem_raw, slot), k, a);
+    }
+    __syncthreads();
+#pragma unroll 1
+    for (int sl = 0; sl < SM::NB; ++sl) {
+      const int64_t ev0 = (b0 + sl) * P::E;
+      if (ev0 >= a.n) break;
+      if (sl > 0) {
+        // the batch body works on the regions of batch 0 (fixed offsets: no pointer that depends on the batch is alive in
+        // its steps): momenta, event indices and weights of batch sl are copied there first (1.7 KB)
+        const unsigned long long* src = reinterpret_cast<const unsigned long long*>(SM::slot_base(smem_raw, sl));
+        SM s0;
+        s0.bind(smem_raw);
+        unsigned long long* dp = reinterpret_cast<unsigned long long*>(s0.pext);
+        unsigned long long* di = reinterpret_cast<unsigned long long*>(SM::evidx(smem_raw));
+        constexpr int NP = (int)(SM::kSlotPext / 8), NI = P::E * 2;
+        for (int t = threadIdx.x; t < NP + NI; t += P::NT) {
+          if (t < NP) { if (t < (int)((size_t)P::E * P::NPAR * 4 * sizeof(T) / 8)) dp[t] = src[t]; }
+          else di[t - NP] = src[t];
+        }
+        __syncthreads();
+      }
+      rc_batch<P, T, TI, MODE>(smem_raw, k, a, ev0, a.n, 0, true);
+      __syncthreads();      // the next batch overwrites the shared memory
     }
   } else {
     rc_batch<P, T, TI, MODE>(smem_raw, k, a, (int64_t)blockIdx.x * P::E, a.n);
@@ -574,7 +633,7 @@ cudaError_t launch_sigmakin_recycle(const mg_process* p, const MeArgs& m, cudaSt
     RcArgs<double> a{(const double*)m.mom, m.n, m.ld, (double*)m.me, (const double*)m.psw, (double*)m.psw_out, (double*)m.evw,
                      (double*)m.hel_out, m.mask, m.seed, m.first, nullptr, nullptr, 0.f, nullptr};
     if (m.hel_out) return launch_rc<P, double, double, M_PERHEL>(p, a, g, s);
-    return m.gen ? launch_rc<P, double, double, M_GEN>(p, a, g, s) : launch_rc<P, double, double, 0>(p, a, g, s);
+    return m.gen ? launch_rc<P, double, double, M_GEN>(p, a, (g + P::GENB - 1) / P::GENB, s) : launch_rc<P, double, double, 0>(p, a, g, s);
   }
   RcArgs<float> a{(const float*)m.mom, m.n, m.ld, (float*)m.me, (const float*)m.psw, (float*)m.psw_out, (float*)m.evw,
                   (float*)m.hel_out, m.mask, m.seed, m.first, m.rescue_list, m.rescue_count, (float)m.rescue_kappa, nullptr};
@@ -583,7 +642,7 @@ cudaError_t launch_sigmakin_recycle(const mg_process* p, const MeArgs& m, cudaSt
     e = cudaMemsetAsync(a.rcount, 0, sizeof(unsigned long long), s);
     if (e != cudaSuccess) return e;
   }
-  e = m.gen ? launch_rc<P, float, float, M_GEN>(p, a, g, s) : launch_rc<P, float, float, 0>(p, a, g, s);
+  e = m.gen ? launch_rc<P, float, float, M_GEN>(p, a, (g + P::GENB32 - 1) / P::GENB32, s) : launch_rc<P, float, float, 0>(p, a, g, s);
   if (e != cudaSuccess || a.rlist == nullptr) return e;
   return m.gen ? launch_rc<P, double, float, M_GATHER | M_GEN>(p, a, 0, s) : launch_rc<P, double, float, M_GATHER>(p, a, 0, s);
 }

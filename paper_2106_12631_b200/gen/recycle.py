@@ -113,18 +113,23 @@ def _closure_key(c):
 #                     combination of the OTHER helicities; |M|^2 counts for the combination and its complement
 #   PRESUM            wavefunctions that enter the same colour-flow sums with the same partner are added up BEFORE the
 #                     inner product: sum_i s_i (R_i . C) = (sum_i s_i R_i) . C, rows first, then columns (_presum)
+#   GENB, GENB32      fused path (momenta generated in the kernel): batches of E events whose momenta a CTA generates up front,
+#                     side by side on different warps, before it runs them one after the other (FP64, FP32): the wait for
+#                     the RAMBO chain is paid once per GENB batches.  g g -> t t~ g FP64: 4.59 -> 4.01 ms per 2^21 events with
+#                     2; slower for FP32 (2.51 -> 2.62) and for g g -> t t~ g g (17.8 -> 21.2: the loop over batches costs
+#                     1.9 KB of spills there)
 #   ORDER             order of the closure classes (indices into the classes sorted by (helicity bits, kind) of their
 #                     half product); None = sorted
 DEFAULTS = {
-    2: dict(E=8, MINB=3, MINB32=3, EG=None, RELAXED='auto', SLOTS=0, BUDGET=240, HOIST=True, HPERM="2301", ORDER=None, FLIP=False, PRESUM=False),
+    2: dict(E=8, MINB=3, MINB32=3, EG=None, RELAXED='auto', SLOTS=0, BUDGET=240, HOIST=True, HPERM="2301", ORDER=None, FLIP=False, PRESUM=False, GENB=1, GENB32=1),
     # FLIP (round 2): one warp (g g -> t t~ g g) / half a warp (g g -> t t~ g) per event, 16 / 32 events per SM.  Without it the
     # tuned shapes were E=4, MINB=4/5, HPERM="23104" and E=4, MINB=2/3, SLOTS=424, HPERM="320145", ORDER=(0, 3, 1, 2)
     # (27.2 ms per 2^20 g g -> t t~ g g events against 17.1 ms; shapes and all 120 / 24 lane orders timed:
     # profiles/r02_h_shapes_and_lane_orders.md)
     # g g -> t t~ g: 96 entries in 6 steps instead of 112 in 4 (BUDGET) so that 32 instead of 24 events fit an SM in FP64, as 2 CTAs
     # of 16 events: 4.39 -> 3.71 ms per 2^21 events (FP32, 4 CTAs: 2.59 -> 2.35); profiles/r02_h_shapes_and_lane_orders.md
-    3: dict(E=16, MINB=2, MINB32=4, EG=None, RELAXED='auto', SLOTS=0, BUDGET=64, HOIST=True, HPERM="2310", ORDER=None, FLIP=True, PRESUM=False),
-    4: dict(E=8, MINB=2, MINB32=3, EG=None, RELAXED='auto', SLOTS=0, BUDGET=96, HOIST=True, HPERM="32410", ORDER=None, FLIP=True, PRESUM=True),
+    3: dict(E=16, MINB=2, MINB32=4, EG=None, RELAXED='auto', SLOTS=0, BUDGET=64, HOIST=True, HPERM="2310", ORDER=None, FLIP=True, PRESUM=False, GENB=2, GENB32=1),
+    4: dict(E=8, MINB=2, MINB32=3, EG=None, RELAXED='auto', SLOTS=0, BUDGET=96, HOIST=True, HPERM="32410", ORDER=None, FLIP=True, PRESUM=True, GENB=1, GENB32=1),
 }
 
 
@@ -618,6 +623,7 @@ def emit(prog):
     w("  static constexpr bool FLIP = %s;" % ("true" if prog.flip else "false"))
     w("  static constexpr int NHEL_FULL = %d, NBITS = %d;" % (1 << npar, npar - (1 if prog.flip else 0)))
     w("  static constexpr int NMOM = %d, NSLOT = %d;" % (len(prog.mom_defs), prog.nslot))
+    w("  static constexpr int GENB = %d, GENB32 = %d;   // batches generated up front by a CTA of the fused path (FP64, FP32)" % (prog.opts["GENB"], prog.opts["GENB32"]))
     # lane bit i of a thread's index within its event carries the helicity of particle hperm[i]: t and t~ in the two
     # lowest bits.  Every order of the free particles was built and timed on B200 (profiles/r02_h_shapes_and_lane_orders.md):
     # 17.1 .. 18.4 ms (g g -> t t~ g g), 4.39 .. 4.54 ms (g g -> t t~ g)
